@@ -213,4 +213,4 @@ def test_matvec_pieces_add_up_and_caller_order(mlp2):
         r = H.aca_block(g, 1e-4)
         ranks.append(r["rank"]); piv_i.append(r["piv_i"]); piv_j.append(r["piv_j"])
     Ur, info = H.matvec(F, 1e-4, replay=(np.array(ranks), np.concatenate(piv_i), np.concatenate(piv_j)))
-    assert info["replay_bad"] == 0 and np.array_equal(Ur, U)
+    assert info["replay_bad"] == 0 and rel_l2(Ur, U) < 1e-14      # (OpenMP sum order)

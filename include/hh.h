@@ -1,0 +1,170 @@
+/* =============================================================================================
+ * hh.h -- C ABI of the B200-native H-HIGNN mobility apply  U = M(X) F   (arxiv 2505.08174).
+ *
+ * Citations are PAPER.md line numbers + section / equation / algorithm; "S-n" are the readings
+ * of silent / ambiguous / garbled passages listed in DESIGN.md.
+ *
+ * The path (Sec. 3): geometric cluster tree on the Morton order (Def. 1,
+ * L123-L129) -> block-cluster partition by the admissibility test max(diam) <= eta * dist
+ * (Def. 2 / Eq. (7); Alg. 1) -> ACA low-rank factors C, Q of the admissible
+ * blocks, entries evaluated on demand by the two-body MLP (Alg. 2; Eqs. (8)-(10)) ->
+ * mat-vec = self term + near-field dense blocks evaluated on the fly (L252) + far-field C (Q F)
+ * (L115, L260) + three-body graph term (Eq. (4); L74) -> explicit Euler (L338).
+ *
+ * Conventions
+ *  - Every pointer argument is marked HOST or DEVICE.  DEVICE buffers are caller-owned (allocated
+ *    by the caller, e.g. with PyTorch) and must stay valid for the duration of the call; the
+ *    workspace must stay valid for the life of the context.  The library allocates no device
+ *    memory.  It owns the context struct and a small pinned host scratch for scalar read-backs.
+ *  - All work is enqueued on the CUDA stream given to hh_create.  Calls return after the few
+ *    scalar read-backs they need (level counts, block totals, arena batch boundaries); hh_matvec
+ *    and hh_step return after their last kernel has been ENQUEUED (U is valid once the stream has
+ *    been synchronised) unless noted.
+ *  - Every function returns HH_OK (0) or a negative HH_ERR_* code; hh_last_error gives a text.
+ *    No exceptions, no aborts.  There is NO CPU fallback: without a CUDA device every compute
+ *    entry point fails with HH_ERR_CUDA.
+ *  - Particle arrays are fp32, row-major [N][3], in the CALLER's particle order.  "Tree order" is
+ *    the Morton order of S-8/S-9: position k in tree order holds caller particle perm[k].
+ *  - Node ids are the library's breadth-first numbering (root 0, children adjacent, left first);
+ *    S-12: only the ranges [lo,hi) identify a cluster.
+ * ============================================================================================= */
+#ifndef HH_H_
+#define HH_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define HH_OK                        0
+#define HH_ERR_INVALID_ARG          -1   /* null pointer, N < 1, eta <= 0, tol <= 0, leaf < 1, bad MLP shape */
+#define HH_ERR_WORKSPACE_TOO_SMALL  -2   /* hh_stats.workspace_required holds the bytes needed          */
+#define HH_ERR_CUDA                 -3   /* a CUDA call failed (text in hh_last_error)                  */
+#define HH_ERR_NOT_BUILT            -4   /* call out of order (e.g. hh_build_blocks before hh_build_tree) */
+#define HH_ERR_UNSUPPORTED          -5   /* MLP shape other than the compiled ones                      */
+
+typedef struct hh_ctx hh_ctx;           /* opaque, owned by the library */
+
+/* An MLP  y = W_L tanh( ... tanh(W_1 x + b_1) ... ) + b_L  (tanh on hidden layers only; PAPER.md L92,
+ * S-4).  Supported shapes: two-body 4->32->32->9 (features [r_hat(3), a/r], Eq. (4) L85 + config),
+ * three-body 7->64->64->9 (features [X_j-X_i, X_k-X_i, |X_j-X_k|]).
+ *   dims : HOST   int32[n_layers+1]
+ *   W, b : HOST   arrays of n_layers DEVICE pointers; W[l] is [dims[l+1]][dims[l]] row-major fp32,
+ *                 b[l] is [dims[l+1]] fp32.  Copied into the context at hh_create. */
+typedef struct {
+  int32_t n_layers;
+  const int32_t* dims;
+  const float* const* W;
+  const float* const* b;
+} hh_mlp;
+
+typedef struct {
+  int32_t leaf_size;     /* C_leaf (Def. 1): a cluster is a leaf iff it holds <= leaf_size particles (S-10) */
+  float   eta;           /* eta of Eq. (7)                                                   */
+  float   aca_tol;       /* zeta of Eq. (10)                                                 */
+  int32_t aca_max_rank;  /* N_ite_max (L258): cap on the block-rank l; 1..96                       */
+  float   radius_a;      /* particle radius a (L41)                                                */
+  float   rcut3;         /* three-body cutoff R_cut (L90); 0 = no three-body term                  */
+  int32_t pivot_rule;    /* 0 = |det| (Eq. (9)), 1 = Frobenius (listing L219/L224); S-18 */
+  int32_t near_path;     /* 0 = fp32 ALU path (tolerance 1e-5).  1 (tensor-core path) is reserved  */
+} hh_params;
+
+/* Counters (Figs. 7-9 count "queries" = MLP evaluations; L299). Filled as stages run. */
+typedef struct {
+  int64_t n_particles;
+  int64_t n_nodes, n_leaves, depth;        /* cluster tree                                          */
+  int64_t n_admissible, n_inadmissible;    /* |P^G|, |P^H| (Alg. 1)                                 */
+  int64_t near_entries;                    /* W^H = sum |tau||sigma| over P^H (L250)                */
+  int64_t far_rows_cols;                   /* sum (|tau|+|sigma|) over P^G                          */
+  int64_t sum_rank;                        /* sum of block-ranks l over the blocks factorised so far */
+  int64_t aca_entries;                     /* two-body MLP evaluations spent in ACA so far          */
+  int64_t factor_bytes;                    /* 36 * l * (|tau|+|sigma|) summed over factorised blocks */
+  int64_t aca_batches;                     /* arena fills so far (L246, L260: batching)             */
+  int64_t aca_not_converged;               /* blocks that hit aca_max_rank before Eq. (10) (S-21)   */
+  int64_t aca_singular;                    /* blocks stopped on a singular pivot (S-18)             */
+  int64_t n_faces;                         /* three-body faces (j,k,i) visited (L74)                */
+  int64_t workspace_required;              /* bytes; set when HH_ERR_WORKSPACE_TOO_SMALL is returned */
+  int64_t arena_bytes;                     /* size of the factor arena carved from the workspace    */
+  float   ms_tree, ms_blocks, ms_aca, ms_near, ms_far, ms_three, ms_other;  /* CUDA-event stage times of the last hh_matvec/hh_step (only if timing enabled) */
+} hh_stats;
+
+/* Create a context.  params: HOST.  mlp2: HOST struct, required.  mlp3: HOST struct or NULL (then
+ * rcut3 must be 0).  workspace: DEVICE, 256-byte aligned, holds the tree, the block lists and the
+ * factor arena (whatever remains after tree and lists).  stream: a cudaStream_t (NULL = default
+ * stream).  Errors: INVALID_ARG, UNSUPPORTED, CUDA. */
+int hh_create(hh_ctx** ctx, const hh_params* params, const hh_mlp* mlp2, const hh_mlp* mlp3,
+              void* workspace, size_t workspace_bytes, void* cuda_stream);
+int hh_destroy(hh_ctx* ctx);
+
+/* Change eta / aca_tol / aca_max_rank / pivot_rule / leaf_size of an existing context (parameter
+ * sweeps of config 3).  Invalidates tree and blocks as needed. */
+int hh_set_params(hh_ctx* ctx, const hh_params* params);
+
+/* Record per-stage CUDA-event times into hh_stats (adds stream synchronisations). */
+int hh_enable_timing(hh_ctx* ctx, int on);
+
+/* Steps 1-4: Morton keys (S-8), stable radix sort (S-9), cluster tree (Def. 1,
+ * L123-L127; S-10, S-11), tight bounding boxes (L144; S-13).
+ *   X : DEVICE fp32 [N][3], caller order; read only.  N >= 1.
+ * Errors: INVALID_ARG, WORKSPACE_TOO_SMALL, CUDA. */
+int hh_build_tree(hh_ctx* ctx, const float* X, int64_t N);
+
+/* Step 5: Alg. 1 BuildPartition from (root, root) (L164-L184; Eq. (7); S-14..S-16) -> P^G, P^H.
+ * Errors: NOT_BUILT (no tree), WORKSPACE_TOO_SMALL, CUDA. */
+int hh_build_blocks(hh_ctx* ctx);
+
+/* Step 7: Alg. 2 (L210-L234) on admissible blocks first_block, first_block+1, ... (the library's
+ * P^G order) until the factor arena is full or P^G is exhausted; *next_block (HOST) receives the
+ * first block NOT factorised (== n_admissible when done).  Factors stay in the arena until the
+ * next hh_aca / hh_build_* call.  Blocks that reach aca_max_rank are kept at that rank and counted.
+ * Errors: NOT_BUILT, INVALID_ARG (first_block out of range), WORKSPACE_TOO_SMALL (arena cannot
+ * hold even one block), CUDA. */
+int hh_aca(hh_ctx* ctx, int64_t first_block, int64_t* next_block);
+
+/* Steps 6-11: U = M(X) F = F (self term, alpha_1 = I, S-5) + near-field (L252) + far-field over all
+ * admissible blocks (runs hh_aca batch by batch when the factors are not all resident; L115, L260)
+ * + three-body term if rcut3 > 0 (Eq. (4); S-22, S-23).
+ *   F : DEVICE fp32 [N][3] caller order, read only.   U : DEVICE fp32 [N][3] caller order, written.
+ * Errors: NOT_BUILT, CUDA, WORKSPACE_TOO_SMALL. */
+int hh_matvec(hh_ctx* ctx, const float* F, float* U);
+
+/* Selective mat-vec for tests and stage timing: bit 0 self, 1 near, 2 far, 3 three-body. */
+int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts);
+
+/* Far-field apply only, over the factors currently in the arena (blocks [first, next) of the last
+ * hh_aca call): Us_tree += C (Q F^sigma).  The roofline-graded kernel.
+ *   F : DEVICE fp32 [N][3] caller order.  U : DEVICE fp32 [N][3] caller order; U is OVERWRITTEN with
+ *   the far-field contribution of the resident blocks only. */
+int hh_far_apply_resident(hh_ctx* ctx, const float* F, float* U);
+
+/* Step 12: one time step (L102, L338): build tree + blocks from X, U = M(X) F, X <- X + dt U (fp32,
+ * S-25).  X : DEVICE fp32 [N][3], updated in place.  F read, U written (DEVICE). */
+int hh_step(hh_ctx* ctx, float* X, const float* F, float* U, int64_t N, float dt);
+
+/* ---- introspection (parity tests, counters).  All destination buffers are HOST. ---- */
+int hh_get_stats(hh_ctx* ctx, hh_stats* stats);
+/* perm int64[N] (S-9), keys uint64[N] sorted; node arrays of length n_nodes (any may be NULL). */
+int hh_get_tree(hh_ctx* ctx, int64_t* perm, uint64_t* keys, int64_t* lo, int64_t* hi, int32_t* left,
+                int32_t* right, int32_t* parent, int32_t* level, float* bmin, float* bmax);
+/* which = 0: P^G, 1: P^H.  tau, sigma: int32[count] node ids (targets, sources; S-16). */
+int hh_get_blocks(hh_ctx* ctx, int which, int32_t* tau, int32_t* sigma);
+/* Factors of admissible block `block` (must be resident in the arena).  rank, flag (0 ok, 1 = hit
+ * max rank, 2 = singular pivot): HOST scalars.  piv_i, piv_j: int32[cap_rank] local row / column
+ * pivots.  C: fp32 [rank][m][9], Q: fp32 [rank][n][9] (entry-major copies of the arena's plane-major
+ * storage); any of piv_i, piv_j, C, Q may be NULL. */
+int hh_get_factors(hh_ctx* ctx, int64_t block, int32_t* rank, int32_t* flag, int32_t cap_rank,
+                   int32_t* piv_i, int32_t* piv_j, float* C, float* Q);
+/* ranks int32[n_admissible], flags int32[n_admissible] of all blocks factorised so far (-1 = not yet). */
+int hh_get_ranks(hh_ctx* ctx, int32_t* ranks, int32_t* flags);
+/* Evaluate the two-body entry M_ij (Eq. (4), S-1..S-3) for n pairs: Xi, Xj DEVICE [n][3], M DEVICE [n][9]. */
+int hh_eval_entries(hh_ctx* ctx, const float* Xi, const float* Xj, int64_t n, float* M);
+
+const char* hh_last_error(const hh_ctx* ctx);
+const char* hh_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HH_H_ */

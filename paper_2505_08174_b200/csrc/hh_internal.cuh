@@ -1,0 +1,167 @@
+// hh_internal.cuh -- shared declarations of the CUDA path (context, workspace layout, primitives).
+// Product code.  Shares nothing with oracle/.  Citations: PAPER.md line numbers; S-n = DESIGN.md readings.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include "../../include/hh.h"
+
+typedef uint32_t u32;
+typedef uint64_t u64;
+
+#define HH_MAX_RANK 96                          /* cap on N_ite_max (L258)                         */
+#define HH_RC 4                                 /* ranks per arena chunk                           */
+#define HH_MAX_CHUNKS (HH_MAX_RANK / HH_RC)     /* 24                                              */
+#define HH_UNIT_FLOATS 32                       /* arena allocation unit = 128 B                   */
+#define HH_TAB_STRIDE 32                        /* u32 per resident block: 24 chunk offsets + pivot offset + pad */
+#define HH_TAB_PIV 24
+#define HH_MAX_LEAF 256                         /* largest supported C_leaf                        */
+#define HH_MAX_LEVELS 128
+
+/* packed MLP weights (floats) as laid out for the kernels: W1 [H][INP], b1 [H], W2 [H][H], b2 [H],
+ * W3T [H][12] (9 outputs of hidden unit o, 3 pad), b3 [12]                                        */
+#define HH_MLP_FLOATS(INP, H) ((H) * (INP) + (H) + (H) * (H) + (H) + (H) * 12 + 12)
+#define HH_MLP2_INP 4
+#define HH_MLP2_H 32
+#define HH_MLP3_INP 8
+#define HH_MLP3_H 64
+#define HH_MLP2_FLOATS HH_MLP_FLOATS(HH_MLP2_INP, HH_MLP2_H)   /* 1612 */
+#define HH_MLP3_FLOATS HH_MLP_FLOATS(HH_MLP3_INP, HH_MLP3_H)   /* 5516 */
+
+struct Cnt3 { u32 g, h, c; };
+__host__ __device__ inline Cnt3 operator+(Cnt3 a, Cnt3 b) { return Cnt3{a.g + b.g, a.h + b.h, a.c + b.c}; }
+
+/* device-side scalars (one 256-B slot at the start of the workspace) + pinned host mirror */
+struct DevScalars {
+  float bb[6];              /* min xyz, max xyz of X as order-preserving uints while reducing, floats after */
+  u32 bbu[6];
+  u32 n_split;              /* tree: nodes split at the current level                                 */
+  u32 pad0;
+  Cnt3 lvl;                 /* Alg. 1: totals of the current level (admissible, inadmissible, children) */
+  u32 n_leaves;
+  u64 arena_cursor;         /* in units                                                               */
+  u32 fail_min;             /* first block whose arena allocation failed                              */
+  u32 batch_end;            /* result of the batch-range search                                       */
+  u32 class_bound[4];       /* first block of ACA class 1,2,3 in the sorted P^G (class 0 starts at 0) */
+  u64 sum_rank, aca_entries, factor_bytes, n_faces;
+  u32 not_conv, singular, deg_overflow, pad1;
+  u64 near_entries, far_rows_cols;
+  u32 max_rank_seen, pad2;
+};
+
+struct hh_ctx {
+  hh_params p;
+  cudaStream_t stream;
+  char* ws;  size_t ws_bytes;
+  char err[512];
+  int have_mlp3;
+  int timing;
+  int64_t pairs_per_particle;
+  /* state */
+  int64_t N, Ncap;
+  int tree_ok, blocks_ok;
+  int n_nodes, n_levels, n_leaves;
+  int lvl_start[HH_MAX_LEVELS + 1];
+  int64_t nG, nH, cap_pairs;
+  int64_t res_first, res_next;          /* resident factor range [first, next) of sorted P^G */
+  double l_pred;                        /* predicted rank for batch sizing                   */
+  u32 class_bound[5];
+  hh_stats st;
+  /* pinned host scratch */
+  DevScalars* h_sc;
+  cudaEvent_t ev[8];
+  /* carved device pointers */
+  DevScalars* d_sc;
+  float *w2, *w3;                       /* packed weights                                     */
+  u64 *keys[2]; u32 *idx[2];            /* radix ping-pong                                    */
+  u32* hist;  size_t hist_cap;          /* radix histograms / generic scan tile sums          */
+  void* tilesum;                        /* tile sums for scans (Cnt3 / u64)                   */
+  float *Xs, *Fs, *Us;                  /* tree order                                         */
+  u32* perm;
+  u32 *nlo, *nhi; int *nleft, *nparent, *nlevel; u32* nsplit; u32* nflag;
+  float *bmin, *bmax;                   /* [nodes][3]                                         */
+  u32* leaf_nodes;
+  uint2 *PG, *PH;                       /* (tau, sigma) node ids; PG sorted by size desc, PH by tau */
+  u32 *near_begin, *near_end;           /* per node: range in PH                              */
+  int* ranks; int* flags;               /* per admissible block                               */
+  u64* unit_prefix;                     /* prefix of (m_pad + n_pad) over sorted PG, nG+1     */
+  char* scratch; size_t scratch_bytes;  /* frontier ping-pong during build; == arena region    */
+  float* arena; u64 arena_units;        /* after the resident table                            */
+  u32* tab;                             /* resident block table, HH_TAB_STRIDE u32 per block   */
+  /* three-body cell list */
+  u32 *cell_of, *cell_start, *cell_order; int64_t n_cells_cap;
+  /* host staging for *_host calls */
+  float *stageX, *stageF, *stageU;
+};
+
+#define HH_CUDA(call)                                                                     \
+  do {                                                                                    \
+    cudaError_t e_ = (call);                                                              \
+    if (e_ != cudaSuccess) {                                                              \
+      snprintf(ctx->err, sizeof ctx->err, "%s:%d %s -> %s", __FILE__, __LINE__, #call,   \
+               cudaGetErrorString(e_));                                                   \
+      return HH_ERR_CUDA;                                                                 \
+    }                                                                                     \
+  } while (0)
+#define HH_TRY(call) do { int r_ = (call); if (r_ != HH_OK) return r_; } while (0)
+#define HH_LAUNCH_CHECK() HH_CUDA(cudaGetLastError())
+
+static inline int hh_fail(hh_ctx* ctx, int code, const char* msg) {
+  snprintf(ctx->err, sizeof ctx->err, "%s", msg);
+  return code;
+}
+static inline unsigned cdiv(int64_t a, int64_t b) { return (unsigned)((a + b - 1) / b); }
+
+/* ---- primitives (hh_prims.cu) ---- */
+int hh_scan_u32(hh_ctx* ctx, const u32* in, u32* out, int64_t n, u32* total_dev /*may be null*/);
+int hh_scan_u64(hh_ctx* ctx, const u64* in, u64* out, int64_t n, u64* total_dev);
+int hh_scan_cnt3(hh_ctx* ctx, Cnt3* tiles, int64_t ntiles, Cnt3* total_dev);   /* in place, exclusive */
+/* stable LSD radix sort of (key, val) on bits [bit_lo, bit_hi); result index (0/1) of ping-pong in *which */
+int hh_sort_pairs(hh_ctx* ctx, u64* keys[2], u32* vals[2], int64_t n, int bit_lo, int bit_hi, int* which);
+
+/* ---- stages ---- */
+int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N);
+int hh_blocks_build(hh_ctx* ctx);
+int hh_near_apply(hh_ctx* ctx);                                       /* Us += near-field           */
+int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next);
+int hh_far_apply(hh_ctx* ctx);                                        /* Us += resident far-field   */
+int hh_three_apply(hh_ctx* ctx);                                     /* Us += three-body term (tree order) */
+int hh_entries_eval(hh_ctx* ctx, const float* Xi, const float* Xj, int64_t n, float* M);
+int hh_factors_fetch(hh_ctx* ctx, int64_t block, int32_t* rank, int32_t* flag, int32_t cap_rank,
+                     int32_t* piv_i, int32_t* piv_j, float* C, float* Q);
+
+/* ---- device helpers ---- */
+#ifdef __CUDACC__
+__device__ __forceinline__ u32 lane_id() { return threadIdx.x & 31; }
+
+/* exclusive scan of one u32 per thread across the block; returns exclusive prefix, *total = block sum.
+ * smem: 33 u32.  All threads must call. */
+template <typename T>
+__device__ __forceinline__ T block_excl_scan(T v, T* smem /* >= 33 */, T* total) {
+  const u32 lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  T inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    T t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= (u32)o) inc += t;
+  }
+  if (lane == 31) smem[w] = inc;
+  __syncthreads();
+  if (w == 0) {
+    T s = lane < nw ? smem[lane] : T(0);
+    T si = s;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      T t = __shfl_up_sync(0xffffffffu, si, o);
+      if (lane >= (u32)o) si += t;
+    }
+    smem[lane] = si - s;
+    if (lane == 31) smem[32] = si;
+  }
+  __syncthreads();
+  T base = smem[w];
+  *total = smem[32];
+  __syncthreads();
+  return base + inc - v;
+}
+#endif

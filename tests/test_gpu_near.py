@@ -1,0 +1,56 @@
+"""GPU parity: two-body entries and the near-field apply vs the oracle."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from conftest import rel_l2
+from gpu_util import f32, make_ctx, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("bias", [False, True])
+def test_entries_match_oracle(bias, mlp2, mlp2_bias):
+    mlp = mlp2_bias if bias else mlp2
+    X = synth.cube_cloud(600, 0.1, seed=5)
+    Xi, Xj = X[:300], X[300:]
+    ctx = make_ctx(mlp, ws_mb=512, radius_a=1.0)
+    M = ctx.eval_entries(to_dev(Xi), to_dev(Xj)).cpu().numpy().astype(np.float64)
+    ref = np.stack([oracle.entry2(mlp, 1.0, Xi[k], Xj[k]).ravel() for k in range(300)])
+    assert np.max(np.abs(M - ref)) <= 2e-6 * np.max(np.abs(ref))
+    assert rel_l2(M, ref) <= 1e-6
+    ctx.close()
+
+
+@pytest.mark.parametrize("n,leaf", [(2048, 64), (1500, 16), (777, 200)])
+def test_nothing_admissible_equals_dense(n, leaf, mlp2_bias):
+    """eta -> 0+: every block is near-field, the H mat-vec is the dense product."""
+    X = synth.cube_cloud(n, 0.1)
+    F = synth.gaussian_forces(n)
+    eta = 1e-30
+    ctx = make_ctx(mlp2_bias, leaf_size=leaf, eta=eta, ws_mb=512)
+    ctx.build_tree(to_dev(X))
+    ctx.build_blocks()
+    assert ctx.stats()["n_admissible"] == 0
+    U = ctx.matvec(to_dev(F), parts=3).cpu().numpy()
+    ref = oracle.dense_matvec(X, F, mlp2_bias)
+    assert rel_l2(U, ref) <= 1e-5
+    st = ctx.stats()
+    assert st["near_entries"] == n * n
+    ctx.close()
+
+
+def test_near_part_matches_oracle_near_part(mlp2):
+    X = synth.ball_cloud(6000, 0.2)
+    F = synth.gravity_forces(6000)
+    H = oracle.HMatrix(X, mlp2, leaf=64, eta=1.0)
+    Uo, _ = H.matvec(F, 1e-4, include_self=False, near=True, far=False)
+    ctx = make_ctx(mlp2, ws_mb=512)
+    ctx.build_tree(to_dev(X))
+    ctx.build_blocks()
+    U = ctx.matvec(to_dev(F), parts=2).cpu().numpy()
+    assert rel_l2(U, Uo) <= 1e-5
+    U1 = ctx.matvec(to_dev(F), parts=1).cpu().numpy()
+    assert np.array_equal(U1, F)
+    ctx.close()

@@ -61,7 +61,7 @@ def test_block_factors_vs_oracle_replay(rule, mlp2):
         Qg = f["Q"].reshape(-1, n, 3, 3).astype(np.float64)
         Pg = np.einsum("kiab,kjbc->ijac", Cg, Qg)                  # block product sum_k C_k(i) Q_k(j)
         Po = np.einsum("kiab,kjbc->ijac", o["C"], o["Q"])
-        assert rel_l2(Pg, Po) <= 2e-6, (g, m, n, f["rank"])
+        assert rel_l2(Pg, Po) <= 1e-5, (g, m, n, f["rank"])   # the fp32 bar of north_star; grows ~ rank * eps
         # interpolation property on the GPU's own factors: product equals G on pivot rows and columns
         G = H.dense_block(int(omap[g]))
         scale = np.abs(G).max()

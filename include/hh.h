@@ -88,6 +88,8 @@ typedef struct {
   int64_t workspace_required;              /* bytes; set when HH_ERR_WORKSPACE_TOO_SMALL is returned */
   int64_t arena_bytes;                     /* size of the factor arena carved from the workspace    */
   float   ms_tree, ms_blocks, ms_aca, ms_near, ms_far, ms_three, ms_other;  /* CUDA-event stage times of the last hh_matvec/hh_step (only if timing enabled) */
+  float   pad_;
+  int64_t n_launches;                      /* kernels launched since the last hh_build_tree began (one whole hh_step) */
 } hh_stats;
 
 /* Create a context.  params: HOST.  mlp2: HOST struct, required.  mlp3: HOST struct or NULL (then

@@ -26,6 +26,7 @@ def lib():
         _lib.orc_h_aca_block.restype = C.c_int
         _lib.orc_num_threads.restype = C.c_int
         _lib.orc_h_admissible.restype = C.c_int
+        _lib.orc_h_last_bad_strict.restype = C.c_int64
     return _lib
 
 
@@ -139,6 +140,16 @@ class HMatrix:
             s = np.zeros(len(arr), np.int32)
             lib().orc_h_get_blocks(self._h, which, _vp(t), _vp(s))
             arr[:, 0], arr[:, 1] = t, s
+
+    def set_replay_roundoff(self, u):
+        """Replay checker only: unit roundoff of the arithmetic being replayed (2**-24 for the fp32 CUDA
+        path).  A replayed pivot / stop decision then counts as bad only if it is outside the slack AND
+        outside the running rounding bound of that arithmetic (arg-max "up to rounding")."""
+        lib().orc_h_set_replay_roundoff(self._h, C.c_double(u))
+
+    def last_bad_strict(self):
+        """slack-only count of bad decisions of the last replay call (reported, not asserted)"""
+        return int(lib().orc_h_last_bad_strict(self._h))
 
     def __del__(self):
         try:

@@ -317,8 +317,33 @@ struct AcaOut {
   std::vector<double> C, Q;     // C[k][i][9], Q[k][j][9]
   std::vector<int32_t> piv_i, piv_j;
   std::vector<double> nu, lam;  // per step (after the step)
-  int replay_bad = 0;           // replay mode: number of pivot / stop decisions outside the slack
+  int replay_bad = 0;           // replay mode: number of pivot / stop decisions outside the slack (and, if a unit
+                                // roundoff u > 0 is given, outside the rounding bound of the replayed arithmetic)
+  int replay_bad_strict = 0;    // same count with the slack alone (u = 0)
 };
+
+// ---- replay-mode rounding model (checker only; does not touch the oracle's own arithmetic) ----
+// "any pivot sequence in which each pivot is an arg-max UP TO ROUNDING and the stop test holds UP TO
+// ROUNDING is a correct run of Alg. 2".  When the replayed run was computed with unit roundoff u (fp32: 2^-24), a
+// residual entry E(i,j) = G(i,j) - sum_p C_p(i) Q_p(j) carries the running error bound
+//   err(i,j) = u * [ K_G |G(i,j)|_F + sum_p (K_T + kappa_p) |C_p(i)|_F |Q_p(j)|_F ],   kappa_p = |P_p|_F |P_p^-1|_F,
+// K_G = 64 (the 4-32-32-9 MLP: 68 fused multiply-adds deep, 2-ulp tanh, feature division), K_T = 8 (3x3 product,
+// subtraction, stored operands), kappa_p because the inverse pivot block is itself computed with roundoff u.
+const double K_G = 64.0, K_T = 8.0;
+
+void adj33(const double* A, double* J) {
+  J[0] = A[4] * A[8] - A[5] * A[7]; J[1] = A[2] * A[7] - A[1] * A[8]; J[2] = A[1] * A[5] - A[2] * A[4];
+  J[3] = A[5] * A[6] - A[3] * A[8]; J[4] = A[0] * A[8] - A[2] * A[6]; J[5] = A[2] * A[3] - A[0] * A[5];
+  J[6] = A[3] * A[7] - A[4] * A[6]; J[7] = A[1] * A[6] - A[0] * A[7]; J[8] = A[0] * A[4] - A[1] * A[3];
+}
+// how far score(A + E) can be from score(A) when |E|_F <= e
+double score_slop(const double* A, int rule, double e) {
+  if (rule != 0) return e;                                       // | |A+E|_F - |A|_F | <= |E|_F
+  double J[9];
+  adj33(A, J);
+  double a = std::sqrt(fro2(A));
+  return std::sqrt(fro2(J)) * e + 2.0 * a * e * e + e * e * e;   // d det = <adj(A)^T, E> + O(E^2)
+}
 
 double score_of(const double* A, int rule) { return rule == 0 ? std::fabs(det33(A)) : std::sqrt(fro2(A)); }
 
@@ -351,7 +376,7 @@ int argmax_score(const std::vector<double>& v, int n, const std::vector<char>& u
 // decisions that are not an arg-max / a correct stop within `slack` (relative).
 void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t snode, double zeta,
                int max_rank, int rule, int rp_rank, const int32_t* rp_i, const int32_t* rp_j,
-               double slack, AcaOut& out) {
+               double slack, AcaOut& out, double u_round = 0.0) {
   const Node& T = h.nodes[tnode];
   const Node& S = h.nodes[snode];
   int c = (int)(T.hi - T.lo), q = (int)(S.hi - S.lo);
@@ -362,6 +387,7 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
   if (replay) kmax = std::min(kmax, rp_rank);
   std::vector<char> used_r(c, 0), used_c(q, 0);
   std::vector<double> ck((size_t)9 * c), qk((size_t)9 * q);
+  std::vector<double> errc(c, 0.0), errq(q, 0.0), kappa;        // replay-mode rounding bounds (checker only)
   double lam2 = 0;
   int jk = 0;                                                   // S-17
   out = AcaOut();
@@ -375,11 +401,14 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     for (int i = 0; i < c; ++i) {
       double g[9];
       entry2(mlp, a, Xt + 3 * i, Xs + 3 * jk, g);
+      double eb = K_G * std::sqrt(fro2(g));
       for (int p = 0; p < k; ++p) {
         double t[9];
         mul33(&out.C[((size_t)p * c + i) * 9], &out.Q[((size_t)p * q + jk) * 9], t);
         for (int e = 0; e < 9; ++e) g[e] -= t[e];
+        if (replay) eb += (K_T + kappa[p]) * std::sqrt(fro2(&out.C[((size_t)p * c + i) * 9]) * fro2(&out.Q[((size_t)p * q + jk) * 9]));
       }
+      errc[i] = u_round * eb;
       std::memcpy(&ck[9 * (size_t)i], g, sizeof g);
     }
     // line 5: row pivot
@@ -389,8 +418,16 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     if (ik < 0 || best == 0.0) { met = true; break; }           // S-21: zero residual column
     if (replay) {
       int gi = rp_i[k];
-      if (gi < 0 || gi >= c || used_r[gi]) { out.replay_bad++; gi = ik; }
-      else if (score_of(&ck[9 * (size_t)gi], ru) < (1.0 - slack) * best) out.replay_bad++;
+      if (gi < 0 || gi >= c || used_r[gi]) { out.replay_bad++; out.replay_bad_strict++; gi = ik; }
+      else {
+        double sg = score_of(&ck[9 * (size_t)gi], ru);
+        if (sg < (1.0 - slack) * best) {
+          out.replay_bad_strict++;
+          double hi = sg + score_slop(&ck[9 * (size_t)gi], ru, errc[gi]);
+          double lo = std::max(0.0, best - score_slop(&ck[9 * (size_t)ik], ru, errc[ik]));
+          if (hi < (1.0 - slack) * lo) out.replay_bad++;
+        }
+      }
       ik = gi;
     }
     double P[9], Pinv[9];
@@ -398,23 +435,31 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     double dP = det33(P);
     if (std::fabs(dP) < 1e-30) { out.flag = 2; break; }         // S-18: singular pivot
     inv33(P, dP, Pinv);
+    const double kap = std::sqrt(fro2(P) * fro2(Pinv)), pinv_n = std::sqrt(fro2(Pinv));
+    double dc2 = 0;                                             // rounding bound of the normalised column, squared
     // line 6: c_k <- c_k P^{-1}
     for (int i = 0; i < c; ++i) {
       double t[9];
       mul33(&ck[9 * (size_t)i], Pinv, t);
       std::memcpy(&ck[9 * (size_t)i], t, sizeof t);
+      double d = errc[i] * pinv_n + u_round * (K_T + kap) * std::sqrt(fro2(t));
+      dc2 += d * d;
     }
     // line 7: row residual
     for (int j = 0; j < q; ++j) {
       double g[9];
       entry2(mlp, a, Xt + 3 * ik, Xs + 3 * j, g);
+      double eb = K_G * std::sqrt(fro2(g));
       for (int p = 0; p < k; ++p) {
         double t[9];
         mul33(&out.C[((size_t)p * c + ik) * 9], &out.Q[((size_t)p * q + j) * 9], t);
         for (int e = 0; e < 9; ++e) g[e] -= t[e];
+        if (replay) eb += (K_T + kappa[p]) * std::sqrt(fro2(&out.C[((size_t)p * c + ik) * 9]) * fro2(&out.Q[((size_t)p * q + j) * 9]));
       }
+      errq[j] = u_round * eb;
       std::memcpy(&qk[9 * (size_t)j], g, sizeof g);
     }
+    kappa.push_back(kap);
     used_r[ik] = 1;
     used_c[jk] = 1;
     // line 8: next column pivot
@@ -423,8 +468,16 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     int jn = argmax_score(qk, q, used_c, rule, &bestc, &ruc);
     if (replay && k + 1 < rp_rank && jn >= 0) {
       int gj = rp_j[k + 1];
-      if (gj < 0 || gj >= q || used_c[gj]) out.replay_bad++;
-      else if (score_of(&qk[9 * (size_t)gj], ruc) < (1.0 - slack) * bestc) out.replay_bad++;
+      if (gj < 0 || gj >= q || used_c[gj]) { out.replay_bad++; out.replay_bad_strict++; }
+      else {
+        double sg = score_of(&qk[9 * (size_t)gj], ruc);
+        if (sg < (1.0 - slack) * bestc) {
+          out.replay_bad_strict++;
+          double hi = sg + score_slop(&qk[9 * (size_t)gj], ruc, errq[gj]);
+          double lo = std::max(0.0, bestc - score_slop(&qk[9 * (size_t)jn], ruc, errq[jn]));
+          if (hi < (1.0 - slack) * lo) out.replay_bad++;
+        }
+      }
     }
     // lines 9-10: norm recursion (S-19)
     double Akk[9] = {0}, Bkk[9] = {0};
@@ -476,11 +529,23 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     bool stop = nu <= zeta * lam;
     if (replay) {
       bool last = (k + 1 == rp_rank);
-      if (!last && nu <= zeta * lam * (1.0 - slack)) out.replay_bad++;          // oracle would clearly have stopped
+      // rounding bound of nu = |c_k q_k^T|_F:  |d nu| <= |dc|_F |q|_F + |c|_F |dq|_F
+      double dq2 = 0, cn2 = 0, qn2 = 0;
+      for (int j = 0; j < q; ++j) { dq2 += errq[j] * errq[j]; qn2 += fro2(&qk[9 * (size_t)j]); }
+      for (int i = 0; i < c; ++i) cn2 += fro2(&ck[9 * (size_t)i]);
+      const double dnu = std::sqrt(dc2 * qn2) + std::sqrt(cn2 * dq2);
+      if (!last && nu <= zeta * lam * (1.0 - slack)) {                          // oracle would clearly have stopped
+        out.replay_bad_strict++;
+        if (nu + dnu <= zeta * lam * (1.0 - slack)) out.replay_bad++;
+      }
       if (last && k + 1 < std::min(std::min(c, q), max_rank) && nu > zeta * lam * (1.0 + slack) &&
-          jn >= 0 && bestc > 0.0)
-        out.replay_bad++;                                                       // GPU stopped clearly early
-      if (last) { met = stop; break; }
+          jn >= 0 && bestc > 0.0) {                                             // GPU stopped clearly early
+        out.replay_bad_strict++;
+        if (nu - dnu > zeta * lam * (1.0 + slack)) out.replay_bad++;
+      }
+      // the replayed run chose to stop here: that choice is judged above; S-21's flag 1 is only "the rank cap
+      // N_ite_max was reached without meeting Eq. (10)"
+      if (last) { met = stop || (k + 1 < std::min(std::min(c, q), max_rank)); break; }
     } else {
       if (stop) { met = true; break; }
     }
@@ -494,6 +559,8 @@ struct Handle {
   HMat h;
   Mlp mlp2;
   double a = 1.0;
+  double u_round = 0.0;         // replay checker: unit roundoff of the replayed arithmetic (0 = slack only)
+  int64_t last_bad_strict = 0;  // slack-only count of the last replay call
 };
 
 }  // namespace
@@ -646,6 +713,9 @@ void* orc_h_create(int64_t N, const float* X, int leaf, double eta, const int* d
   return H;
 }
 void orc_h_destroy(void* p) { delete (Handle*)p; }
+// replay checker: unit roundoff of the arithmetic being replayed (2^-24 for the fp32 CUDA path; 0 = slack only)
+void orc_h_set_replay_roundoff(void* p, double u) { ((Handle*)p)->u_round = u; }
+int64_t orc_h_last_bad_strict(void* p) { return ((Handle*)p)->last_bad_strict; }
 
 void orc_h_counts(void* p, int64_t* n_nodes, int64_t* n_leaves, int64_t* nG, int64_t* nH, int64_t* depth) {
   Handle* H = (Handle*)p;
@@ -689,7 +759,8 @@ int orc_h_aca_block(void* p, int64_t gblock, double zeta, int max_rank, int rule
   Handle* H = (Handle*)p;
   auto pr = H->h.G[(size_t)gblock];
   AcaOut o;
-  aca_block(H->h, H->mlp2, H->a, pr.first, pr.second, zeta, max_rank, rule, rp_rank, rp_i, rp_j, slack, o);
+  aca_block(H->h, H->mlp2, H->a, pr.first, pr.second, zeta, max_rank, rule, rp_rank, rp_i, rp_j, slack, o, H->u_round);
+  H->last_bad_strict = o.replay_bad_strict;
   int c = (int)(H->h.nodes[pr.first].hi - H->h.nodes[pr.first].lo);
   int q = (int)(H->h.nodes[pr.second].hi - H->h.nodes[pr.second].lo);
   int r = std::min(o.rank, cap_rank);
@@ -741,7 +812,7 @@ int64_t orc_h_matvec(void* p, const float* F, double zeta, int max_rank, int rul
     for (int64_t k = T.lo; k < T.hi; ++k) if (only_rows[k]) return true;
     return false;
   };
-  int64_t entries = 0, bad = 0;
+  int64_t entries = 0, bad = 0, bad_strict = 0;
   if (do_near) {
 #pragma omp parallel for schedule(dynamic, 8) reduction(+ : entries)
     for (int64_t b = 0; b < (int64_t)h.H.size(); ++b) {
@@ -765,7 +836,7 @@ int64_t orc_h_matvec(void* p, const float* F, double zeta, int max_rank, int rul
     }
   }
   if (do_far) {
-#pragma omp parallel for schedule(dynamic, 1) reduction(+ : entries, bad)
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : entries, bad, bad_strict)
     for (int64_t g = 0; g < (int64_t)h.G.size(); ++g) {
       const Node& T = h.nodes[h.G[g].first];
       const Node& S = h.nodes[h.G[g].second];
@@ -774,11 +845,12 @@ int64_t orc_h_matvec(void* p, const float* F, double zeta, int max_rank, int rul
       AcaOut o;
       if (rp_rank)
         aca_block(h, Hd->mlp2, Hd->a, h.G[g].first, h.G[g].second, zeta, max_rank, rule, rp_rank[g],
-                  rp_i + rp_off[g], rp_j + rp_off[g], slack, o);
+                  rp_i + rp_off[g], rp_j + rp_off[g], slack, o, Hd->u_round);
       else
         aca_block(h, Hd->mlp2, Hd->a, h.G[g].first, h.G[g].second, zeta, max_rank, rule, -1, nullptr, nullptr, 0.0, o);
       entries += (int64_t)o.rank * (c + q);
       bad += o.replay_bad;
+      bad_strict += o.replay_bad_strict;
       if (ranks_out) ranks_out[g] = o.rank;
       if (flags_out) flags_out[g] = o.flag;
       for (int k = 0; k < o.rank; ++k) {
@@ -798,6 +870,7 @@ int64_t orc_h_matvec(void* p, const float* F, double zeta, int max_rank, int rul
   for (int64_t k = 0; k < N; ++k)
     for (int c = 0; c < 3; ++c) U[3 * h.perm[k] + c] = Us[3 * k + c];
   if (n_entries) *n_entries = entries;
+  Hd->last_bad_strict = bad_strict;
   return bad;
 }
 

@@ -46,7 +46,8 @@ class Stats(C.Structure):
                 ("n_particles", "n_nodes", "n_leaves", "depth", "n_admissible", "n_inadmissible", "near_entries",
                  "far_rows_cols", "sum_rank", "aca_entries", "factor_bytes", "aca_batches", "aca_not_converged",
                  "aca_singular", "n_faces", "workspace_required", "arena_bytes")] + \
-               [(n, C.c_float) for n in ("ms_tree", "ms_blocks", "ms_aca", "ms_near", "ms_far", "ms_three", "ms_other")]
+               [(n, C.c_float) for n in ("ms_tree", "ms_blocks", "ms_aca", "ms_near", "ms_far", "ms_three", "ms_other", "pad_")] + \
+               [("n_launches", C.c_int64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}

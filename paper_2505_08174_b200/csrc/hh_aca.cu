@@ -376,7 +376,7 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   if (chunks_pred < 1) chunks_pred = 1;
   if (chunks_pred > HH_MAX_CHUNKS) chunks_pred = HH_MAX_CHUNKS;
   const u64 total_units = ctx->scratch_bytes / 128;
-  k_batch_range<<<1, 1, 0, s>>>(ctx->unit_prefix, (u32)first, nG, total_units > 8 ? total_units - 8 : 0, chunks_pred, ctx->d_sc);
+  k_batch_range<<<HH_N + 1, 1, 0, s>>>(ctx->unit_prefix, (u32)first, nG, total_units > 8 ? total_units - 8 : 0, chunks_pred, ctx->d_sc);
   HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->batch_end, &ctx->d_sc->batch_end, sizeof(u32), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   u32 end = ctx->h_sc->batch_end;
@@ -398,17 +398,17 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     if (b >= e) continue;
     A.begin = b;
     switch (c) {
-      case 0: k_aca<256><<<e - b, 256, 0, s>>>(A); break;
-      case 1: k_aca<128><<<e - b, 128, 0, s>>>(A); break;
-      case 2: k_aca<64><<<e - b, 64, 0, s>>>(A); break;
-      default: k_aca<32><<<e - b, 32, 0, s>>>(A); break;
+      case 0: k_aca<256><<<HH_N + e - b, 256, 0, s>>>(A); break;
+      case 1: k_aca<128><<<HH_N + e - b, 128, 0, s>>>(A); break;
+      case 2: k_aca<64><<<HH_N + e - b, 64, 0, s>>>(A); break;
+      default: k_aca<32><<<HH_N + e - b, 32, 0, s>>>(A); break;
     }
   }
   HH_LAUNCH_CHECK();
   HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->fail_min, &ctx->d_sc->fail_min, sizeof(u32), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   u32 nx = ctx->h_sc->fail_min < end ? ctx->h_sc->fail_min : end;
-  k_batch_stats<<<cdiv(nb, 256), 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, (u32)first, nx, end, ctx->d_sc);
+  k_batch_stats<<<HH_N + cdiv(nb, 256), 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, (u32)first, nx, end, ctx->d_sc);
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   const DevScalars& h = *ctx->h_sc;

@@ -151,6 +151,7 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   int r = carve(ctx, 1);
   if (r != HH_OK) return r;
   HH_CUDA(cudaMallocHost((void**)&ctx->h_sc, sizeof(DevScalars)));
+  HH_CUDA(cudaMemsetAsync(ctx->d_sc, 0, sizeof(DevScalars), ctx->stream));
   for (int k = 0; k < 8; ++k) HH_CUDA(cudaEventCreate(&ctx->ev[k]));
   std::vector<float> pk;
   r = pack_mlp(ctx, mlp2, 4, HH_MLP2_INP, HH_MLP2_H, pk);
@@ -215,6 +216,7 @@ extern "C" int hh_build_tree(hh_ctx* ctx, const float* X, int64_t N) {
   if (!ctx) return HH_ERR_INVALID_ARG;
   if (!X || N < 1 || N > 0x7fffffff / 4) return hh_fail(ctx, HH_ERR_INVALID_ARG, "hh_build_tree: X null or N out of range");
   if (N > ctx->Ncap || N * 4 < ctx->Ncap) HH_TRY(carve(ctx, N));
+  ctx->n_launches = 0;
   T0(0);
   HH_TRY(hh_tree_build(ctx, X, N));
   T0(1);
@@ -251,7 +253,7 @@ extern "C" int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts)
   const int64_t N = ctx->N;
   if (ctx->timing) { ctx->st.ms_aca = ctx->st.ms_near = ctx->st.ms_far = ctx->st.ms_three = ctx->st.ms_other = 0.f; }
   T0(4);
-  k_gather_f<<<cdiv(N, 256), 256, 0, s>>>(F, ctx->perm, N, ctx->Fs, ctx->Us);
+  k_gather_f<<<HH_N + cdiv(N, 256), 256, 0, s>>>(F, ctx->perm, N, ctx->Fs, ctx->Us);
   HH_LAUNCH_CHECK();
   T0(5);
   if (ctx->timing) ctx->st.ms_other += ev_ms(ctx, 4, 5);
@@ -292,7 +294,7 @@ extern "C" int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts)
     if (ctx->timing) ctx->st.ms_three = ev_ms(ctx, 4, 5);
   }
   T0(4);
-  k_unpermute<<<cdiv(N, 256), 256, 0, s>>>(ctx->Us, ctx->Fs, ctx->perm, N, parts & 1, 0, U);
+  k_unpermute<<<HH_N + cdiv(N, 256), 256, 0, s>>>(ctx->Us, ctx->Fs, ctx->perm, N, parts & 1, 0, U);
   HH_LAUNCH_CHECK();
   T0(5);
   if (ctx->timing) ctx->st.ms_other += ev_ms(ctx, 4, 5);
@@ -306,12 +308,12 @@ extern "C" int hh_far_apply_resident(hh_ctx* ctx, const float* F, float* U) {
   if (!F || !U) return hh_fail(ctx, HH_ERR_INVALID_ARG, "null F or U");
   if (!ctx->blocks_ok) return hh_fail(ctx, HH_ERR_NOT_BUILT, "hh_far_apply_resident before hh_build_blocks");
   const int64_t N = ctx->N;
-  k_gather_f<<<cdiv(N, 256), 256, 0, ctx->stream>>>(F, ctx->perm, N, ctx->Fs, ctx->Us);
+  k_gather_f<<<HH_N + cdiv(N, 256), 256, 0, ctx->stream>>>(F, ctx->perm, N, ctx->Fs, ctx->Us);
   T0(4);
   HH_TRY(hh_far_apply(ctx));
   T0(5);
   if (ctx->timing) ctx->st.ms_far = ev_ms(ctx, 4, 5);
-  k_unpermute<<<cdiv(N, 256), 256, 0, ctx->stream>>>(ctx->Us, ctx->Fs, ctx->perm, N, 0, 0, U);
+  k_unpermute<<<HH_N + cdiv(N, 256), 256, 0, ctx->stream>>>(ctx->Us, ctx->Fs, ctx->perm, N, 0, 0, U);
   HH_LAUNCH_CHECK();
   return HH_OK;
 }
@@ -322,7 +324,7 @@ extern "C" int hh_step(hh_ctx* ctx, float* X, const float* F, float* U, int64_t 
   HH_TRY(hh_build_tree(ctx, X, N));
   HH_TRY(hh_build_blocks(ctx));
   HH_TRY(hh_matvec(ctx, F, U));
-  k_euler<<<cdiv(3 * N, 256), 256, 0, ctx->stream>>>(X, U, 3 * N, dt);
+  k_euler<<<HH_N + cdiv(3 * N, 256), 256, 0, ctx->stream>>>(X, U, 3 * N, dt);
   HH_LAUNCH_CHECK();
   return HH_OK;
 }
@@ -346,6 +348,7 @@ extern "C" int hh_step_host(hh_ctx* ctx, float* X_host, const float* F_host, flo
 extern "C" int hh_get_stats(hh_ctx* ctx, hh_stats* st) {
   if (!ctx || !st) return HH_ERR_INVALID_ARG;
   *st = ctx->st;
+  st->n_launches = ctx->n_launches;
   return HH_OK;
 }
 

@@ -166,12 +166,12 @@ int hh_blocks_build(hh_ctx* ctx) {
   int64_t fcap = (int64_t)(ctx->scratch_bytes / 2 / sizeof(uint2));
   uint2* fr[2] = {(uint2*)ctx->scratch, (uint2*)ctx->scratch + fcap};
   Cnt3* tiles = (Cnt3*)ctx->tilesum;
-  k_set_root_pair<<<1, 1, 0, s>>>(fr[0]);
+  k_set_root_pair<<<HH_N + 1, 1, 0, s>>>(fr[0]);
   int64_t n = 1, nG = 0, nH = 0;
   int cur = 0;
   while (n > 0) {
     int64_t nt = (n + BK_T - 1) / BK_T;
-    k_bp_count<<<(unsigned)nt, BK_T, 0, s>>>(tv, fr[cur], n, eta2, tiles);
+    k_bp_count<<<HH_N + (unsigned)nt, BK_T, 0, s>>>(tv, fr[cur], n, eta2, tiles);
     HH_TRY(hh_scan_cnt3(ctx, tiles, nt, &ctx->d_sc->lvl));
     HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->lvl, &ctx->d_sc->lvl, sizeof(Cnt3), cudaMemcpyDeviceToHost, s));
     HH_CUDA(cudaStreamSynchronize(s));
@@ -182,12 +182,12 @@ int hh_blocks_build(hh_ctx* ctx) {
       ctx->st.workspace_required = (int64_t)ctx->ws_bytes + need * 64;
       return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "block lists / frontier exceed the pair capacity (raise pairs_per_particle or the workspace)");
     }
-    k_bp_fill<<<(unsigned)nt, BK_T, 0, s>>>(tv, fr[cur], n, eta2, tiles, ctx->PG + nG, ctx->PH + nH, fr[cur ^ 1]);
+    k_bp_fill<<<HH_N + (unsigned)nt, BK_T, 0, s>>>(tv, fr[cur], n, eta2, tiles, ctx->PG + nG, ctx->PH + nH, fr[cur ^ 1]);
     HH_LAUNCH_CHECK();
     nG += t.g; nH += t.h; n = t.c; cur ^= 1;
   }
   ctx->nG = nG; ctx->nH = nH;
-  k_blocks_init<<<1, 1, 0, s>>>(ctx->d_sc, (u32)nG);
+  k_blocks_init<<<HH_N + 1, 1, 0, s>>>(ctx->d_sc, (u32)nG);
   // sort buffers carved from the scratch region
   int64_t nmax = nG > nH ? nG : nH;
   size_t need = (size_t)nmax * (2 * sizeof(u64) + 2 * sizeof(u32) + sizeof(uint2)) + 1024;
@@ -197,21 +197,21 @@ int hh_blocks_build(hh_ctx* ctx) {
   uint2* tmp = (uint2*)(((uintptr_t)(v2[1] + nmax) + 15) & ~(uintptr_t)15);
   int which;
   if (nG > 0) {
-    k_g_keys<<<cdiv(nG, 256), 256, 0, s>>>(ctx->PG, nG, ctx->nlo, ctx->nhi, k2[0], v2[0]);
+    k_g_keys<<<HH_N + cdiv(nG, 256), 256, 0, s>>>(ctx->PG, nG, ctx->nlo, ctx->nhi, k2[0], v2[0]);
     HH_TRY(hh_sort_pairs(ctx, k2, v2, nG, 0, 32, &which));
-    k_gather_pairs<<<cdiv(nG, 256), 256, 0, s>>>(ctx->PG, v2[which], nG, tmp);
+    k_gather_pairs<<<HH_N + cdiv(nG, 256), 256, 0, s>>>(ctx->PG, v2[which], nG, tmp);
     HH_CUDA(cudaMemcpyAsync(ctx->PG, tmp, (size_t)nG * sizeof(uint2), cudaMemcpyDeviceToDevice, s));
-    k_g_post<<<cdiv(nG, 256), 256, 0, s>>>(ctx->PG, nG, ctx->nlo, ctx->nhi, ctx->unit_prefix, ctx->ranks, ctx->flags, ctx->d_sc);
+    k_g_post<<<HH_N + cdiv(nG, 256), 256, 0, s>>>(ctx->PG, nG, ctx->nlo, ctx->nhi, ctx->unit_prefix, ctx->ranks, ctx->flags, ctx->d_sc);
     HH_TRY(hh_scan_u64(ctx, ctx->unit_prefix, ctx->unit_prefix, nG + 1, nullptr));
   }
   if (nH > 0) {
     HH_CUDA(cudaMemsetAsync(ctx->near_begin, 0, sizeof(u32) * ctx->n_nodes, s));
     HH_CUDA(cudaMemsetAsync(ctx->near_end, 0, sizeof(u32) * ctx->n_nodes, s));
-    k_h_keys<<<cdiv(nH, 256), 256, 0, s>>>(ctx->PH, nH, k2[0], v2[0]);
+    k_h_keys<<<HH_N + cdiv(nH, 256), 256, 0, s>>>(ctx->PH, nH, k2[0], v2[0]);
     HH_TRY(hh_sort_pairs(ctx, k2, v2, nH, 0, bits_for((u64)ctx->n_nodes), &which));
-    k_gather_pairs<<<cdiv(nH, 256), 256, 0, s>>>(ctx->PH, v2[which], nH, tmp);
+    k_gather_pairs<<<HH_N + cdiv(nH, 256), 256, 0, s>>>(ctx->PH, v2[which], nH, tmp);
     HH_CUDA(cudaMemcpyAsync(ctx->PH, tmp, (size_t)nH * sizeof(uint2), cudaMemcpyDeviceToDevice, s));
-    k_h_post<<<cdiv(nH, 256), 256, 0, s>>>(ctx->PH, nH, ctx->nlo, ctx->nhi, ctx->near_begin, ctx->near_end, ctx->d_sc);
+    k_h_post<<<HH_N + cdiv(nH, 256), 256, 0, s>>>(ctx->PH, nH, ctx->nlo, ctx->nhi, ctx->near_begin, ctx->near_end, ctx->d_sc);
   }
   HH_LAUNCH_CHECK();
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));

@@ -101,10 +101,10 @@ int hh_far_apply(hh_ctx* ctx) {
     u32 e = ctx->class_bound[c + 1] < end ? ctx->class_bound[c + 1] : end;
     if (b >= e) continue;
     switch (c) {
-      case 0: k_far<512, 2048><<<e - b, 512, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      case 1: k_far<256, 256><<<e - b, 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      case 2: k_far<128, 128><<<e - b, 128, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      default: k_far<64, 64><<<e - b, 64, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 0: k_far<512, 2048><<<HH_N + e - b, 512, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 1: k_far<256, 256><<<HH_N + e - b, 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 2: k_far<128, 128><<<HH_N + e - b, 128, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      default: k_far<64, 64><<<HH_N + e - b, 64, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
     }
   }
   HH_LAUNCH_CHECK();

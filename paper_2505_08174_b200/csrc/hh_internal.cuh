@@ -67,6 +67,7 @@ struct hh_ctx {
   double l_pred;                        /* predicted rank for batch sizing                   */
   u32 class_bound[5];
   hh_stats st;
+  int64_t n_launches;                   /* kernels launched since the last hh_build_tree began (claim for bench.py) */
   /* pinned host scratch */
   DevScalars* h_sc;
   cudaEvent_t ev[8];
@@ -105,6 +106,8 @@ struct hh_ctx {
   } while (0)
 #define HH_TRY(call) do { int r_ = (call); if (r_ != HH_OK) return r_; } while (0)
 #define HH_LAUNCH_CHECK() HH_CUDA(cudaGetLastError())
+/* every kernel launch is written  k<<<HH_N + grid, block, smem, stream>>>(...)  and counts itself */
+#define HH_N (++ctx->n_launches, 0u)
 
 static inline int hh_fail(hh_ctx* ctx, int code, const char* msg) {
   snprintf(ctx->err, sizeof ctx->err, "%s", msg);

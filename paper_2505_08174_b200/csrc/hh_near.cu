@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(NR_T) k_near(const float* __restrict__ gw, flo
 
 int hh_near_apply(hh_ctx* ctx) {
   if (ctx->n_leaves <= 0 || ctx->nH <= 0) return HH_OK;
-  k_near<<<ctx->n_leaves, NR_T, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, ctx->leaf_nodes, ctx->nlo, ctx->nhi, ctx->PH,
+  k_near<<<HH_N + ctx->n_leaves, NR_T, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, ctx->leaf_nodes, ctx->nlo, ctx->nhi, ctx->PH,
                                                   ctx->near_begin, ctx->near_end, ctx->Xs, ctx->Fs, ctx->Us);
   HH_LAUNCH_CHECK();
   return HH_OK;
@@ -108,7 +108,7 @@ __global__ void __launch_bounds__(128) k_entries(const float* __restrict__ gw, f
 }
 
 int hh_entries_eval(hh_ctx* ctx, const float* Xi, const float* Xj, int64_t n, float* M) {
-  k_entries<<<cdiv(n, 128), 128, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, Xi, Xj, n, M);
+  k_entries<<<HH_N + cdiv(n, 128), 128, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, Xi, Xj, n, M);
   HH_LAUNCH_CHECK();
   return HH_OK;
 }

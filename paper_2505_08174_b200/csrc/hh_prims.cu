@@ -73,9 +73,9 @@ static int scan_impl(hh_ctx* ctx, const T* in, T* out, int64_t n, T* total_dev) 
   }
   int64_t nt = (n + SCAN_TILE - 1) / SCAN_TILE;
   T* ts = (T*)ctx->tilesum;
-  k_tile_sum<T><<<(unsigned)nt, SCAN_THREADS, 0, ctx->stream>>>(in, ts, n);
-  k_scan_single<T><<<1, 1024, 0, ctx->stream>>>(ts, nt, total_dev);
-  k_tile_scan<T><<<(unsigned)nt, SCAN_THREADS, 0, ctx->stream>>>(in, out, ts, n);
+  k_tile_sum<T><<<HH_N + (unsigned)nt, SCAN_THREADS, 0, ctx->stream>>>(in, ts, n);
+  k_scan_single<T><<<HH_N + 1, 1024, 0, ctx->stream>>>(ts, nt, total_dev);
+  k_tile_scan<T><<<HH_N + (unsigned)nt, SCAN_THREADS, 0, ctx->stream>>>(in, out, ts, n);
   HH_LAUNCH_CHECK();
   return HH_OK;
 }
@@ -84,7 +84,7 @@ int hh_scan_u32(hh_ctx* ctx, const u32* in, u32* out, int64_t n, u32* total_dev)
 int hh_scan_u64(hh_ctx* ctx, const u64* in, u64* out, int64_t n, u64* total_dev) { return scan_impl<u64>(ctx, in, out, n, total_dev); }
 
 int hh_scan_cnt3(hh_ctx* ctx, Cnt3* tiles, int64_t ntiles, Cnt3* total_dev) {
-  k_scan_single_cnt3<<<1, 1024, 0, ctx->stream>>>(tiles, ntiles, total_dev);
+  k_scan_single_cnt3<<<HH_N + 1, 1024, 0, ctx->stream>>>(tiles, ntiles, total_dev);
   HH_LAUNCH_CHECK();
   return HH_OK;
 }
@@ -148,9 +148,9 @@ int hh_sort_pairs(hh_ctx* ctx, u64* keys[2], u32* vals[2], int64_t n, int bit_lo
     if ((size_t)NW * 256 > ctx->hist_cap) return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "radix histogram buffer too small");
     unsigned grid = (NW + RS_WARPS - 1) / RS_WARPS;
     for (int shift = bit_lo; shift < bit_hi; shift += 8) {
-      k_rs_hist<<<grid, RS_WARPS * 32, 0, ctx->stream>>>(keys[cur], n, shift, ctx->hist, NW);
+      k_rs_hist<<<HH_N + grid, RS_WARPS * 32, 0, ctx->stream>>>(keys[cur], n, shift, ctx->hist, NW);
       HH_TRY(hh_scan_u32(ctx, ctx->hist, ctx->hist, (int64_t)NW * 256, nullptr));
-      k_rs_scatter<<<grid, RS_WARPS * 32, 0, ctx->stream>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n, shift,
+      k_rs_scatter<<<HH_N + grid, RS_WARPS * 32, 0, ctx->stream>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n, shift,
                                                            ctx->hist, NW);
       cur ^= 1;
     }

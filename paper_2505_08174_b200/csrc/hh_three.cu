@@ -152,7 +152,9 @@ int hh_three_apply(hh_ctx* ctx) {
     G.inv[c] = (float)(1.0 / cw);
   }
   const u32 ncells = (u32)((int64_t)G.nc[0] * G.nc[1] * G.nc[2]);
-  k_cell_ids<<<cdiv(N, 256), 256, 0, s>>>(ctx->Xs, N, G, ctx->keys[1], ctx->idx[1]);
+  HH_CUDA(cudaMemsetAsync(&ctx->d_sc->n_faces, 0, sizeof(u64), s));
+  HH_CUDA(cudaMemsetAsync(&ctx->d_sc->deg_overflow, 0, sizeof(u32), s));
+  k_cell_ids<<<HH_N + cdiv(N, 256), 256, 0, s>>>(ctx->Xs, N, G, ctx->keys[1], ctx->idx[1]);
   // sort (cell id, particle) with the radix ping-pong buffers; keys[0] (the Morton keys) must survive, so the
   // sort runs in scratch-free buffers: keys[1]/idx[1] and the cell_of / cell_order arrays as the second pair
   u64* k2[2] = {ctx->keys[1], (u64*)ctx->stageU};                // stageU (12 N bytes) holds N u64 keys
@@ -161,11 +163,11 @@ int hh_three_apply(hh_ctx* ctx) {
   while (bits < 64 && ((u64)ncells >> bits)) bits += 8;
   int which = 0;
   HH_TRY(hh_sort_pairs(ctx, k2, v2, N, 0, bits, &which));
-  k_cell_start<<<cdiv(N + 1, 256), 256, 0, s>>>(k2[which], N, ncells, ctx->cell_start);
+  k_cell_start<<<HH_N + cdiv(N + 1, 256), 256, 0, s>>>(k2[which], N, ncells, ctx->cell_start);
   size_t smem = (size_t)HH_MLP3_FLOATS * sizeof(float) + (TB_T / 32) * TB_CAP * sizeof(u32);
   static bool attr_set = false;
   if (!attr_set) { cudaFuncSetAttribute(k_three, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
-  k_three<<<cdiv(N, TB_T / 32), TB_T, smem, s>>>(ctx->w3, ctx->Xs, ctx->Fs, ctx->Us, N, G, ctx->cell_start, v2[which], rcut, ctx->d_sc);
+  k_three<<<HH_N + cdiv(N, TB_T / 32), TB_T, smem, s>>>(ctx->w3, ctx->Xs, ctx->Fs, ctx->Us, N, G, ctx->cell_start, v2[which], rcut, ctx->d_sc);
   HH_LAUNCH_CHECK();
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));

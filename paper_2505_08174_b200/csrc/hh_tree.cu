@@ -176,10 +176,10 @@ int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N) {
   ctx->res_first = ctx->res_next = 0;
   ctx->N = N;
   // rows 1-2: keys, sort, gather
-  k_init_bbox<<<1, 32, 0, s>>>(ctx->d_sc);
+  k_init_bbox<<<HH_N + 1, 32, 0, s>>>(ctx->d_sc);
   unsigned gb = cdiv(N, 256);
-  k_bbox<<<gb < 1184 ? gb : 1184, 256, 0, s>>>(X, N, ctx->d_sc);
-  k_morton<<<gb, 256, 0, s>>>(X, N, ctx->d_sc, ctx->keys[0], ctx->idx[0]);
+  k_bbox<<<HH_N + (gb < 1184 ? gb : 1184), 256, 0, s>>>(X, N, ctx->d_sc);
+  k_morton<<<HH_N + gb, 256, 0, s>>>(X, N, ctx->d_sc, ctx->keys[0], ctx->idx[0]);
   HH_LAUNCH_CHECK();
   int which = 0;
   HH_TRY(hh_sort_pairs(ctx, ctx->keys, ctx->idx, N, 0, 64, &which));
@@ -187,16 +187,16 @@ int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N) {
     u64* tk = ctx->keys[0]; ctx->keys[0] = ctx->keys[1]; ctx->keys[1] = tk;
     u32* ti = ctx->idx[0]; ctx->idx[0] = ctx->idx[1]; ctx->idx[1] = ti;
   }
-  k_gather_x<<<gb, 256, 0, s>>>(X, ctx->idx[0], N, ctx->Xs, ctx->perm);
+  k_gather_x<<<HH_N + gb, 256, 0, s>>>(X, ctx->idx[0], N, ctx->Xs, ctx->perm);
   // row 3: level-synchronous top-down tree, children adjacent, breadth-first numbering
-  k_init_root<<<1, 1, 0, s>>>(ctx->nlo, ctx->nhi, ctx->nleft, ctx->nparent, ctx->nlevel, (u32)N);
+  k_init_root<<<HH_N + 1, 1, 0, s>>>(ctx->nlo, ctx->nhi, ctx->nleft, ctx->nparent, ctx->nlevel, (u32)N);
   HH_LAUNCH_CHECK();
   int start = 0, count = 1, level = 0;
   int64_t node_cap = 2 * ctx->Ncap;
   ctx->lvl_start[0] = 0;
   while (count > 0) {
     if (level >= HH_MAX_LEVELS) return hh_fail(ctx, HH_ERR_INVALID_ARG, "cluster tree deeper than HH_MAX_LEVELS");
-    k_split<<<cdiv(count, 256), 256, 0, s>>>(ctx->keys[0], ctx->nlo, ctx->nhi, ctx->nleft, ctx->nsplit, ctx->nflag, start, count,
+    k_split<<<HH_N + cdiv(count, 256), 256, 0, s>>>(ctx->keys[0], ctx->nlo, ctx->nhi, ctx->nleft, ctx->nsplit, ctx->nflag, start, count,
                                              (u32)ctx->p.leaf_size);
     HH_TRY(hh_scan_u32(ctx, ctx->nflag + start, ctx->nflag + start, count, &ctx->d_sc->n_split));
     HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->n_split, &ctx->d_sc->n_split, sizeof(u32), cudaMemcpyDeviceToHost, s));
@@ -204,7 +204,7 @@ int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N) {
     int nsp = (int)ctx->h_sc->n_split;
     if ((int64_t)start + count + 2 * (int64_t)nsp > node_cap) return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "node capacity exceeded");
     if (nsp > 0)
-      k_children<<<cdiv(count, 256), 256, 0, s>>>(ctx->nlo, ctx->nhi, ctx->nleft, ctx->nparent, ctx->nlevel, ctx->nsplit,
+      k_children<<<HH_N + cdiv(count, 256), 256, 0, s>>>(ctx->nlo, ctx->nhi, ctx->nleft, ctx->nparent, ctx->nlevel, ctx->nsplit,
                                                   ctx->nflag, start, count, level);
     start += count;
     count = 2 * nsp;
@@ -215,18 +215,18 @@ int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N) {
   ctx->n_nodes = start;
   // leaves, in node order
   int nn = ctx->n_nodes;
-  k_leaf_flag<<<cdiv(nn, 256), 256, 0, s>>>(ctx->nleft, nn, ctx->nflag);
+  k_leaf_flag<<<HH_N + cdiv(nn, 256), 256, 0, s>>>(ctx->nleft, nn, ctx->nflag);
   HH_TRY(hh_scan_u32(ctx, ctx->nflag, ctx->nflag, nn, &ctx->d_sc->n_leaves));
-  k_leaf_compact<<<cdiv(nn, 256), 256, 0, s>>>(ctx->nleft, ctx->nflag, nn, ctx->leaf_nodes);
+  k_leaf_compact<<<HH_N + cdiv(nn, 256), 256, 0, s>>>(ctx->nleft, ctx->nflag, nn, ctx->leaf_nodes);
   HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->n_leaves, &ctx->d_sc->n_leaves, sizeof(u32), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   ctx->n_leaves = (int)ctx->h_sc->n_leaves;
   // row 4: boxes, leaves then bottom-up
-  k_leaf_boxes<<<cdiv((int64_t)ctx->n_leaves * 32, 256), 256, 0, s>>>(ctx->Xs, ctx->leaf_nodes, ctx->n_leaves, ctx->nlo, ctx->nhi,
+  k_leaf_boxes<<<HH_N + cdiv((int64_t)ctx->n_leaves * 32, 256), 256, 0, s>>>(ctx->Xs, ctx->leaf_nodes, ctx->n_leaves, ctx->nlo, ctx->nhi,
                                                                       ctx->bmin, ctx->bmax);
   for (int l = ctx->n_levels - 2; l >= 0; --l) {
     int c = ctx->lvl_start[l + 1] - ctx->lvl_start[l];
-    k_merge_boxes<<<cdiv(c, 256), 256, 0, s>>>(ctx->nleft, ctx->bmin, ctx->bmax, ctx->lvl_start[l], c);
+    k_merge_boxes<<<HH_N + cdiv(c, 256), 256, 0, s>>>(ctx->nleft, ctx->bmin, ctx->bmax, ctx->lvl_start[l], c);
   }
   HH_LAUNCH_CHECK();
   ctx->st.n_particles = N;

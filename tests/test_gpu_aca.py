@@ -2,7 +2,8 @@
 
 ACA factors are not unique (SURVEY 8(c) "several results are correct"): the oracle re-runs Alg. 2 in fp64
 with the GPU's pivots and rank (replay) and checks that every GPU decision is an arg-max / a correct stop
-within 1e-3 relative slack; what is unique given the pivots -- each rank term C_k(i) Q_k(j), the block
+within 1e-3 relative slack or within the running fp32 rounding bound of the residual it was taken on
+(oracle replay checker); what is unique given the pivots -- each rank term C_k(i) Q_k(j), the block
 product and the mat-vec -- is compared element by element."""
 import numpy as np
 import pytest
@@ -43,6 +44,7 @@ def test_block_factors_vs_oracle_replay(rule, mlp2):
     X = synth.cube_cloud(3000, 0.1)
     zeta = 1e-4
     H = oracle.HMatrix(X, mlp2, leaf=32, eta=2.0)
+    H.set_replay_roundoff(2.0 ** -24)
     ctx = setup(X, mlp2, leaf_size=32, eta=2.0, aca_tol=zeta, pivot_rule=rule)
     assert ctx.aca(0) == H.nG
     tr = ctx.get_tree()
@@ -50,7 +52,7 @@ def test_block_factors_vs_oracle_replay(rule, mlp2):
     omap = map_blocks_to_oracle(tr, t, s, H)
     sizes = (tr["hi"][t] - tr["lo"][t]) * (tr["hi"][s] - tr["lo"][s])
     pick = list(np.argsort(-sizes)[:6]) + list(np.argsort(sizes)[:6]) + list(range(0, len(t), max(1, len(t) // 12)))
-    bad_total = 0
+    bad_total = strict_total = 0
     for g in pick:
         m, n = int(tr["hi"][t[g]] - tr["lo"][t[g]]), int(tr["hi"][s[g]] - tr["lo"][s[g]])
         f = ctx.get_factors(int(g), m, n)
@@ -67,6 +69,7 @@ def test_block_factors_vs_oracle_replay(rule, mlp2):
         scale = np.abs(G).max()
         assert np.abs(Pg[f["piv_i"]] - G[f["piv_i"]]).max() <= 2e-5 * scale
         assert np.abs(Pg[:, f["piv_j"]] - G[:, f["piv_j"]]).max() <= 2e-5 * scale
+    print("rule", rule, "decisions outside the 1e-3 slack alone:", strict_total, "outside slack and fp32 rounding:", bad_total)
     assert bad_total == 0
 
 
@@ -81,7 +84,8 @@ def test_matvec_vs_oracle(name, gen, leaf, eta, zeta, mlp2):
     N = len(X)
     F = synth.gaussian_forces(N)
     H = oracle.HMatrix(X, mlp2, leaf=leaf, eta=f32(eta))
-    ctx = setup(X, mlp2, leaf_size=leaf, eta=eta, aca_tol=zeta)
+    H.set_replay_roundoff(2.0 ** -24)
+    ctx = setup(X, mlp2, leaf_size=leaf, eta=eta, aca_tol=zeta, ws_mb=8192)
     U = ctx.matvec(to_dev(F)).cpu().numpy()
     tr = ctx.get_tree()
     st = ctx.stats()
@@ -91,7 +95,8 @@ def test_matvec_vs_oracle(name, gen, leaf, eta, zeta, mlp2):
     # (1) the bar: GPU vs oracle with the GPU's pivots
     assert rel_l2(U, Uo) <= 1e-5
     assert np.array_equal(info["flags"], flags)
-    assert info["replay_bad"] <= max(1, H.nG // 200)           # near-ties beyond the 1e-3 slack are rare
+    print(name, "replay decisions outside slack alone:", H.last_bad_strict(), "outside slack and fp32 rounding:", info["replay_bad"])
+    assert info["replay_bad"] == 0
     # (2) reported: free-running oracle
     Uf, finfo = H.matvec(F, f32(zeta))
     print(name, "free-run rel L2", rel_l2(U, Uf), "rank diff blocks", int(np.sum(finfo["ranks"] != info["ranks"])))
@@ -109,7 +114,7 @@ def test_matvec_vs_oracle(name, gen, leaf, eta, zeta, mlp2):
 def test_arena_batches_give_same_result(mlp2):
     X = synth.cube_cloud(6000, 0.1)
     F = synth.gaussian_forces(6000)
-    big = setup(X, mlp2, leaf_size=16, eta=2.0, aca_tol=1e-4)
+    big = setup(X, mlp2, leaf_size=16, eta=2.0, aca_tol=1e-4, ws_mb=8192)
     U1 = big.matvec(to_dev(F)).cpu().numpy()
     st1 = big.stats()
     assert st1["aca_batches"] == 1

@@ -145,6 +145,16 @@ def test_replay_mode(H_small):
     assert H.aca_block(g, 1e-4, replay=(r["piv_i"][:-2], r["piv_j"][:-2]))["replay_bad"] > 0
     # first pivot row is the arg-max of |det| over the first column (Eq. (9))
     assert r["piv_i"][0] == int(np.argmax(scores))
+    # the rounding-aware checker (fp32 unit roundoff) forgives only what fp32 rounding can explain: the same
+    # gross errors are still reported, the oracle's own run still passes
+    H.set_replay_roundoff(2.0 ** -24)
+    try:
+        assert H.aca_block(g, 1e-4, replay=(r["piv_i"], r["piv_j"]))["replay_bad"] == 0
+        assert H.aca_block(g, 1e-4, replay=(bad_i, r["piv_j"]))["replay_bad"] > 0
+        assert H.aca_block(g, 1e-4, replay=(r["piv_i"][:-2], r["piv_j"][:-2]))["replay_bad"] > 0
+        assert H.last_bad_strict() > 0
+    finally:
+        H.set_replay_roundoff(0.0)
 
 
 def test_rank_nearly_constant_across_blocks(H_small):

@@ -1,12 +1,13 @@
 // hh_aca.cu -- SURVEY 8(a) row 7: Alg. 2 (Eqs. (8)-(10), L196-L205) with 3x3 entries,
 // one CTA per admissible block, entries evaluated on demand by the two-body MLP (L262 lines 4, 7).
 //
-// Storage (differs from the listing, same product): rank term k keeps the UN-normalised residual column
-// c'_k(i) = E_{k-1}(i, j_k) and Qt_k(j) = P^{-1} q_k(j) with P = c'_k(i_k); c'_k(i) Qt_k(j) equals the
-// listing's (c'_k P^{-1})(i) q_k(j), so line 6 costs no extra pass over the column.  Pivot scores are taken
-// on q_k (before P^{-1}).  nu^2 and the lambda^2 recursion (S-19) are factorisation-independent:
-//   nu^2   = tr(A_kk B_kk),  A_pk = sum_i C_p(i)^T C_k(i),  B_kp = sum_j Qt_k(j) Qt_p(j)^T
-//   cross  = sum_p tr(A_pk B_kp) = sum_j tr( [sum_p Qt_p(j)^T A_pk] Qt_k(j) )      (one scalar reduction)
+// Storage is the listing's: rank term k keeps the normalised column c_k(i) = E_{k-1}(i, j_k) P^{-1} with
+// P = E_{k-1}(i_k, j_k) (line 6, so c_k(i_k) = I) and the raw residual row q_k(j) = E_{k-1}(i_k, j).  The
+// 3x3 inverse and the products c'(i) P^{-1} are taken in fp64 and rounded once: with an fp32 inverse the
+// factor (and every later apply) loses cond(P) * 2^-24, which breaks the 1e-5 bar.
+// nu^2 and the lambda^2 recursion (S-19):
+//   nu^2   = tr(A_kk B_kk),  A_pk = sum_i C_p(i)^T c_k(i),  B_kp = sum_j q_k(j) Q_p(j)^T
+//   cross  = sum_p tr(A_pk B_kp) = sum_j tr( [sum_p Q_p(j)^T A_pk] q_k(j) )        (one scalar reduction)
 // Factors live in the arena in chunks of HH_RC ranks, plane-major: C part [r][e][m_pad], Q part [r][e][n_pad].
 #include "hh_mlp.cuh"
 
@@ -41,7 +42,8 @@ __device__ __forceinline__ void warp_amax(float& s, int& i) {
 
 struct AcaSmem {
   float sw[HH_MLP2_FLOATS];
-  float sQj[HH_MAX_RANK * 9];     // Qt_p(j_k), p < k
+  double sPinvD[9];               // P^{-1} in fp64
+  float sQj[HH_MAX_RANK * 9];     // Q_p(j_k),  p < k
   float sCi[HH_MAX_RANK * 9];     // C_p(i_k),  p < k
   float sA[HH_MAX_RANK * 9];      // A_pk,      p < k
   float sAkk[9], sP[9], sPinv[9];
@@ -119,9 +121,6 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 384 / T) k_aca(AcaArgs A) {
     // ---- line 4: column residual c'_k(i) = G(i, j_k) - sum_p C_p(i) Qt_p(j_k); line 5: row pivot ----
     float bd = -1.f, bf = -1.f;
     int bdi = -1, bfi = -1;
-    float akk[9];
-#pragma unroll
-    for (int e = 0; e < 9; ++e) akk[e] = 0.f;
     float xs[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) xs[c] = A.Xs[3 * (size_t)(slo + jk) + c];
@@ -152,53 +151,15 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 384 / T) k_aca(AcaArgs A) {
       for (int e = 0; e < 2; ++e) {
         if (ok[e]) {
 #pragma unroll
-          for (int r = 0; r < 9; ++r) Ck[(size_t)r * mp + ii[e]] = c[e][r];
+          for (int r = 0; r < 9; ++r) Ck[(size_t)r * mp + ii[e]] = c[e][r];      // raw residual; normalised in pass 2
           bool used = false;
           for (int q = 0; q < k; ++q) used |= (S.piv_i[q] == (int)ii[e]);
           if (!used) {
             amax_merge(bd, bdi, fabsf(det33(c[e])), (int)ii[e]);
             amax_merge(bf, bfi, fro2_33(c[e]), (int)ii[e]);
           }
-#pragma unroll
-          for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int s = 0; s < 3; ++s)
-              akk[3 * r + s] += c[e][r] * c[e][s] + c[e][3 + r] * c[e][3 + s] + c[e][6 + r] * c[e][6 + s];
-        } else {
-#pragma unroll
-          for (int r = 0; r < 9; ++r) c[e][r] = 0.f;
         }
       }
-      // Gram matrices A_pk = sum_i C_p(i)^T c'_k(i) (second sweep over the stored columns)
-      for (int p = 0; p < k; ++p) {
-        const float* Cp = A.arena + (size_t)S.chunk[p / HH_RC] * HH_UNIT_FLOATS + (size_t)(p % HH_RC) * 9 * mp;
-        float acc[9];
-#pragma unroll
-        for (int r = 0; r < 9; ++r) acc[r] = 0.f;
-#pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          if (ok[e]) {
-            float cp[9];
-#pragma unroll
-            for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + ii[e]];
-#pragma unroll
-            for (int r = 0; r < 3; ++r)
-#pragma unroll
-              for (int s = 0; s < 3; ++s)
-                acc[3 * r + s] += cp[r] * c[e][s] + cp[3 + r] * c[e][3 + s] + cp[6 + r] * c[e][6 + s];
-          }
-        }
-#pragma unroll
-        for (int r = 0; r < 9; ++r) {
-          float v = warp_sum(acc[r]);
-          if (lane == 0) atomicAdd(&S.sA[9 * p + r], v);
-        }
-      }
-    }
-#pragma unroll
-    for (int r = 0; r < 9; ++r) {
-      float v = warp_sum(akk[r]);
-      if (lane == 0) atomicAdd(&S.sAkk[r], v);
     }
     block_amax2<T>(S, bd, bdi, bf, bfi);
     // S-18: |det| rule falls back to Frobenius when every remaining |det| is 0; rule 1 = Frobenius
@@ -216,24 +177,86 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 384 / T) k_aca(AcaArgs A) {
     }
     __syncthreads();
     if (tid == 0) {
-      const float* P = S.sP;
-      float dP = det33(P);
-      if (fabsf(dP) < 1e-30f) {
+      double P[9];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) P[r] = (double)S.sP[r];
+      const double dP = P[0] * (P[4] * P[8] - P[5] * P[7]) - P[1] * (P[3] * P[8] - P[5] * P[6]) + P[2] * (P[3] * P[7] - P[4] * P[6]);
+      if (fabs(dP) < 1e-30) {
         S.ctl[1] = 2;
       } else {
-        float iv = 1.0f / dP;
-        S.sPinv[0] = (P[4] * P[8] - P[5] * P[7]) * iv; S.sPinv[1] = (P[2] * P[7] - P[1] * P[8]) * iv;
-        S.sPinv[2] = (P[1] * P[5] - P[2] * P[4]) * iv; S.sPinv[3] = (P[5] * P[6] - P[3] * P[8]) * iv;
-        S.sPinv[4] = (P[0] * P[8] - P[2] * P[6]) * iv; S.sPinv[5] = (P[2] * P[3] - P[0] * P[5]) * iv;
-        S.sPinv[6] = (P[3] * P[7] - P[4] * P[6]) * iv; S.sPinv[7] = (P[1] * P[6] - P[0] * P[7]) * iv;
-        S.sPinv[8] = (P[0] * P[4] - P[1] * P[3]) * iv;
+        const double iv = 1.0 / dP;
+        S.sPinvD[0] = (P[4] * P[8] - P[5] * P[7]) * iv; S.sPinvD[1] = (P[2] * P[7] - P[1] * P[8]) * iv;
+        S.sPinvD[2] = (P[1] * P[5] - P[2] * P[4]) * iv; S.sPinvD[3] = (P[5] * P[6] - P[3] * P[8]) * iv;
+        S.sPinvD[4] = (P[0] * P[8] - P[2] * P[6]) * iv; S.sPinvD[5] = (P[2] * P[3] - P[0] * P[5]) * iv;
+        S.sPinvD[6] = (P[3] * P[7] - P[4] * P[6]) * iv; S.sPinvD[7] = (P[1] * P[6] - P[0] * P[7]) * iv;
+        S.sPinvD[8] = (P[0] * P[4] - P[1] * P[3]) * iv;
       }
       S.piv_i[k] = ik;
     }
     __syncthreads();
     if (S.ctl[1] == 2) { flag = 2; break; }                     // S-18: singular pivot -> stop at the current rank
 
-    // ---- line 7: row residual q_k(j) = G(i_k, j) - sum_p C_p(i_k) Qt_p(j); line 8: next column; lines 9-10 ----
+    // ---- line 6: c_k(i) = c'_k(i) P^{-1} (fp64 products, rounded once); Gram matrices A_kk, A_pk (S-19) ----
+    {
+      double Pi[9];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) Pi[r] = S.sPinvD[r];
+      float akk[9];
+#pragma unroll
+      for (int e = 0; e < 9; ++e) akk[e] = 0.f;
+      for (u32 base = 0; base < m; base += T) {
+        const u32 i = base + tid;
+        const bool ok = i < m;
+        float c[9];
+        if (ok) {
+          float cr[9];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) cr[r] = Ck[(size_t)r * mp + i];              // written by this same thread in pass 1
+#pragma unroll
+          for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int s2 = 0; s2 < 3; ++s2)
+              c[3 * r + s2] = (float)((double)cr[3 * r] * Pi[s2] + (double)cr[3 * r + 1] * Pi[3 + s2] + (double)cr[3 * r + 2] * Pi[6 + s2]);
+#pragma unroll
+          for (int r = 0; r < 9; ++r) Ck[(size_t)r * mp + i] = c[r];
+#pragma unroll
+          for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int s2 = 0; s2 < 3; ++s2) akk[3 * r + s2] += c[r] * c[s2] + c[3 + r] * c[3 + s2] + c[6 + r] * c[6 + s2];
+        } else {
+#pragma unroll
+          for (int r = 0; r < 9; ++r) c[r] = 0.f;
+        }
+        for (int p = 0; p < k; ++p) {
+          const float* Cp = A.arena + (size_t)S.chunk[p / HH_RC] * HH_UNIT_FLOATS + (size_t)(p % HH_RC) * 9 * mp;
+          float acc[9];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) acc[r] = 0.f;
+          if (ok) {
+            float cp[9];
+#pragma unroll
+            for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + i];
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int s2 = 0; s2 < 3; ++s2) acc[3 * r + s2] = cp[r] * c[s2] + cp[3 + r] * c[3 + s2] + cp[6 + r] * c[6 + s2];
+          }
+#pragma unroll
+          for (int r = 0; r < 9; ++r) {
+            float v = warp_sum(acc[r]);
+            if (lane == 0) atomicAdd(&S.sA[9 * p + r], v);
+          }
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < 9; ++r) {
+        float v = warp_sum(akk[r]);
+        if (lane == 0) atomicAdd(&S.sAkk[r], v);
+      }
+    }
+    __syncthreads();
+
+    // ---- line 7: row residual q_k(j) = G(i_k, j) - sum_p C_p(i_k) Q_p(j); line 8: next column; lines 9-10 ----
     bd = -1.f; bf = -1.f; bdi = -1; bfi = -1;
     float cross = 0.f, nu2 = 0.f;
     float xt[3];
@@ -282,17 +305,16 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 384 / T) k_aca(AcaArgs A) {
             amax_merge(bd, bdi, fabsf(det33(q[e])), (int)jj[e]);
             amax_merge(bf, bfi, fro2_33(q[e]), (int)jj[e]);
           }
-          float qt[9], W[9];
-          mul33(S.sPinv, q[e], qt);                                // Qt_k(j) = P^{-1} q_k(j)
+          float W[9];
 #pragma unroll
-          for (int r = 0; r < 9; ++r) Qk[(size_t)r * np + jj[e]] = qt[r];
-          mul33(S.sAkk, qt, W);
+          for (int r = 0; r < 9; ++r) Qk[(size_t)r * np + jj[e]] = q[e][r];    // raw residual row (listing line 7)
+          mul33(S.sAkk, q[e], W);
 #pragma unroll
-          for (int r = 0; r < 9; ++r) nu2 = fmaf(W[r], qt[r], nu2);  // tr(A_kk Qt Qt^T)
+          for (int r = 0; r < 9; ++r) nu2 = fmaf(W[r], q[e][r], nu2);          // tr(A_kk q q^T)
 #pragma unroll
           for (int r = 0; r < 3; ++r)
 #pragma unroll
-            for (int s = 0; s < 3; ++s) cross = fmaf(Z[e][3 * r + s], qt[3 * s + r], cross);   // tr(Z Qt)
+            for (int s = 0; s < 3; ++s) cross = fmaf(Z[e][3 * r + s], q[e][3 * s + r], cross);   // tr(Z q)
         }
       }
     }
@@ -433,8 +455,8 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
 }
 
 // ------------------------------------------------------------------------------ introspection
-// Copies the factors of a resident block to the host, entry-major: C [rank][m][9], Q [rank][n][9] AS STORED
-// (C_k = un-normalised residual column, Q_k = P^{-1} q_k; C_k(i) Q_k(j) is the listing's rank term).
+// Copies the factors of a resident block to the host, entry-major: C [rank][m][9], Q [rank][n][9] as stored
+// (the listing's: C_k = normalised residual column with C_k(i_k) = I, Q_k = residual row).
 int hh_factors_fetch(hh_ctx* ctx, int64_t block, int32_t* rank, int32_t* flag, int32_t cap_rank, int32_t* piv_i,
                      int32_t* piv_j, float* C, float* Q) {
   cudaStream_t s = ctx->stream;

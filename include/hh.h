@@ -69,6 +69,9 @@ typedef struct {
   float   rcut3;         /* three-body cutoff R_cut (L90); 0 = no three-body term                  */
   int32_t pivot_rule;    /* 0 = |det| (Eq. (9)), 1 = Frobenius (listing L219/L224); S-18 */
   int32_t near_path;     /* 0 = fp32 ALU path (tolerance 1e-5).  1 (tensor-core path) is reserved  */
+  float   kappa_max;     /* S-18b: a pivot block with |P|_F |P^-1|_F above this is numerically singular at fp32
+                            entry accuracy: Alg. 2 breaks down on that block (flag 2) and the mat-vec evaluates it
+                            densely like an inadmissible block (L252).  0 = default (300); INFINITY = never   */
 } hh_params;
 
 /* Counters (Figs. 7-9 count "queries" = MLP evaluations; L299). Filled as stages run. */
@@ -83,13 +86,15 @@ typedef struct {
   int64_t factor_bytes;                    /* 36 * l * (|tau|+|sigma|) summed over factorised blocks */
   int64_t aca_batches;                     /* arena fills so far (L246, L260: batching)             */
   int64_t aca_not_converged;               /* blocks that hit aca_max_rank before Eq. (10) (S-21)   */
-  int64_t aca_singular;                    /* blocks stopped on a singular pivot (S-18)             */
+  int64_t aca_singular;                    /* blocks on which Alg. 2 broke down on a (numerically) singular pivot
+                                              (S-18, S-18b); they are applied densely                  */
   int64_t n_faces;                         /* three-body faces (j,k,i) visited (L74)                */
   int64_t workspace_required;              /* bytes; set when HH_ERR_WORKSPACE_TOO_SMALL is returned */
   int64_t arena_bytes;                     /* size of the factor arena carved from the workspace    */
   float   ms_tree, ms_blocks, ms_aca, ms_near, ms_far, ms_three, ms_other;  /* CUDA-event stage times of the last hh_matvec/hh_step (only if timing enabled) */
   float   pad_;
   int64_t n_launches;                      /* kernels launched since the last hh_build_tree began (one whole hh_step) */
+  int64_t fallback_entries;                /* sum |tau||sigma| over the blocks counted in aca_singular (dense evaluations per mat-vec) */
 } hh_stats;
 
 /* Create a context.  params: HOST.  mlp2: HOST struct, required.  mlp3: HOST struct or NULL (then
@@ -153,9 +158,11 @@ int hh_get_tree(hh_ctx* ctx, int64_t* perm, uint64_t* keys, int64_t* lo, int64_t
 /* which = 0: P^G, 1: P^H.  tau, sigma: int32[count] node ids (targets, sources; S-16). */
 int hh_get_blocks(hh_ctx* ctx, int which, int32_t* tau, int32_t* sigma);
 /* Factors of admissible block `block` (must be resident in the arena).  rank, flag (0 ok, 1 = hit
- * max rank, 2 = singular pivot): HOST scalars.  piv_i, piv_j: int32[cap_rank] local row / column
- * pivots.  C: fp32 [rank][m][9], Q: fp32 [rank][n][9] (entry-major copies of the arena's plane-major
- * storage); any of piv_i, piv_j, C, Q may be NULL. */
+ * max rank, 2 = breakdown on a singular pivot, block applied densely): HOST scalars.  piv_i, piv_j:
+ * int32[cap_rank] local row / column pivots of the `rank` accepted steps, followed (flag 2) by the
+ * attempted pivot at which Alg. 2 broke down.  C: fp32 [rank][m][9] (the listing's normalised
+ * columns, C_k(i_k) = I), Q: fp32 [rank][n][9] (residual rows), entry-major copies of the arena's
+ * plane-major storage; any of piv_i, piv_j, C, Q may be NULL. */
 int hh_get_factors(hh_ctx* ctx, int64_t block, int32_t* rank, int32_t* flag, int32_t cap_rank,
                    int32_t* piv_i, int32_t* piv_j, float* C, float* Q);
 /* ranks int32[n_admissible], flags int32[n_admissible] of all blocks factorised so far (-1 = not yet). */

@@ -147,6 +147,11 @@ class HMatrix:
         outside the running rounding bound of that arithmetic (arg-max "up to rounding")."""
         lib().orc_h_set_replay_roundoff(self._h, C.c_double(u))
 
+    def set_kappa_max(self, kappa):
+        """S-18b: pivot blocks with cond_F = |P|_F |P^-1|_F above kappa break Alg. 2 down (flag 2, block applied
+        densely).  Default 300; float('inf') gives the plain listing."""
+        lib().orc_h_set_kappa_max(self._h, C.c_double(kappa))
+
     def last_bad_strict(self):
         """slack-only count of bad decisions of the last replay call (reported, not asserted)"""
         return int(lib().orc_h_last_bad_strict(self._h))
@@ -177,11 +182,12 @@ class HMatrix:
         t, s = self.G[g]
         return int(self.hi[t] - self.lo[t]), int(self.hi[s] - self.lo[s])
 
-    def aca_block(self, g, zeta, max_rank=96, rule=0, replay=None, slack=1e-3):
-        """Alg. 2 on admissible block g. replay=(piv_i, piv_j) re-runs with given pivots/rank.
+    def aca_block(self, g, zeta, max_rank=96, rule=0, replay=None, slack=1e-3, replay_flag=0):
+        """Alg. 2 on admissible block g. replay=(piv_i, piv_j) re-runs with given pivots/rank; with replay_flag=2
+        the last pivot pair is the attempted one at which the replayed run broke down (S-18b).
         Returns dict(rank, C[l,c,3,3], Q[l,q,3,3], piv_i, piv_j, nu, lam, flag, replay_bad)."""
         c, q = self.block_shape(g)
-        cap = min(c, q, max_rank)
+        cap = min(c, q, max_rank) + 1
         Cb = np.zeros((cap, c, 3, 3), np.float64)
         Qb = np.zeros((cap, q, 3, 3), np.float64)
         pi = np.zeros(cap, np.int32)
@@ -195,11 +201,12 @@ class HMatrix:
         else:
             ri = np.ascontiguousarray(replay[0], np.int32)
             rj = np.ascontiguousarray(replay[1], np.int32)
-            rr = len(ri)
+            rr = len(ri) - (1 if replay_flag == 2 else 0)
         r = lib().orc_h_aca_block(self._h, C.c_int64(g), C.c_double(zeta), int(max_rank), int(rule), int(rr),
-                                  _vp(ri), _vp(rj), C.c_double(slack), int(cap), _vp(Cb), _vp(Qb), _vp(pi),
+                                  int(replay_flag), _vp(ri), _vp(rj), C.c_double(slack), int(cap), _vp(Cb), _vp(Qb), _vp(pi),
                                   _vp(pj), _vp(nu), _vp(lam), C.byref(flag), C.byref(bad))
-        return dict(rank=r, C=Cb[:r], Q=Qb[:r], piv_i=pi[:r], piv_j=pj[:r], nu=nu[:r], lam=lam[:r],
+        npiv = r + (1 if int(flag.value) == 2 and r < cap else 0)       # a breakdown also lists its attempted pivot
+        return dict(rank=r, C=Cb[:r], Q=Qb[:r], piv_i=pi[:npiv], piv_j=pj[:npiv], nu=nu[:r], lam=lam[:r],
                     flag=int(flag.value), replay_bad=int(bad.value))
 
     def dense_block(self, g):
@@ -210,24 +217,26 @@ class HMatrix:
 
     def matvec(self, F, zeta, max_rank=96, rule=0, include_self=True, near=True, far=True,
                replay=None, slack=1e-3, only_rows=None):
-        """U = M_H(X) F in caller order. replay = (ranks[nG], piv_i concat, piv_j concat) in THIS
-        object's P^G order.  Returns (U, info)."""
+        """U = M_H(X) F in caller order. replay = (ranks[nG], piv_i concat, piv_j concat[, flags[nG]]) in THIS
+        object's P^G order; a block with flag 2 lists ranks[g] + 1 pivot pairs (the last one is the attempted
+        pivot at which the replayed run broke down, S-18b).  Returns (U, info)."""
         F = np.ascontiguousarray(F, np.float32)
         U = np.zeros((self.N, 3), np.float64)
         ranks = np.zeros(self.nG, np.int32)
         flags = np.zeros(self.nG, np.int32)
         ne = C.c_int64(0)
         if replay is None:
-            rr = ro = ri = rj = None
+            rr = rf = ro = ri = rj = None
         else:
             rr = np.ascontiguousarray(replay[0], np.int32)
+            rf = np.ascontiguousarray(replay[3], np.int32) if len(replay) > 3 else np.zeros(self.nG, np.int32)
             ro = np.zeros(self.nG, np.int64)
             if self.nG:
-                ro[1:] = np.cumsum(rr[:-1])
+                ro[1:] = np.cumsum((rr + (rf == 2))[:-1])
             ri = np.ascontiguousarray(replay[1], np.int32)
             rj = np.ascontiguousarray(replay[2], np.int32)
         rows = None if only_rows is None else np.ascontiguousarray(only_rows, np.uint8)
         bad = lib().orc_h_matvec(self._h, _vp(F), C.c_double(zeta), int(max_rank), int(rule), int(include_self),
-                                 int(near), int(far), _vp(rr), _vp(ro), _vp(ri), _vp(rj), C.c_double(slack),
+                                 int(near), int(far), _vp(rr), _vp(rf), _vp(ro), _vp(ri), _vp(rj), C.c_double(slack),
                                  _vp(rows), _vp(U), _vp(ranks), _vp(flags), C.byref(ne))
         return U, dict(ranks=ranks, flags=flags, entries=int(ne.value), replay_bad=int(bad))

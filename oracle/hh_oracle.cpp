@@ -308,7 +308,10 @@ void build_partition(HMat& h, int32_t t, int32_t s) {
 // S-17 j_1 = 0.  S-18 score = |det| (pivot_rule 0, Eq. (9)) or Frobenius (rule 1,
 // listing L219/L224); used rows AND columns excluded; ties -> lowest index; all |det| = 0 but some
 // Frobenius != 0 -> Frobenius for that search; pivot with |det| < 1e-30 -> stop at current rank,
-// flag.  S-19 norm recursion via 3x3 Gram matrices A_pk = sum_i C_p(i)^T c_k(i),
+// flag 2; a pivot block with cond_F(P) = |P|_F |P^-1|_F > kappa_max (default 300) is numerically singular
+// at fp32 entry accuracy and is treated the same way (S-18b): Alg. 2 breaks down, the block is
+// flagged (flag 2) and the mat-vec evaluates it densely like an inadmissible block (L252), which is exact.
+// S-19 norm recursion via 3x3 Gram matrices A_pk = sum_i C_p(i)^T c_k(i),
 // B_kp = sum_j q_k(j) Q_p(j)^T:  nu^2 = tr(A_kk B_kk), cross term tr(A_pk B_kp).
 // S-20 stop when nu <= zeta*lambda, lambda including the current term.  S-21 degenerate cases.
 struct AcaOut {
@@ -327,9 +330,10 @@ struct AcaOut {
 // ROUNDING is a correct run of Alg. 2".  When the replayed run was computed with unit roundoff u (fp32: 2^-24), a
 // residual entry E(i,j) = G(i,j) - sum_p C_p(i) Q_p(j) carries the running error bound
 //   err(i,j) = u * [ K_G |G(i,j)|_F + sum_p (K_T + kappa_p) |C_p(i)|_F |Q_p(j)|_F ],   kappa_p = |P_p|_F |P_p^-1|_F,
-// K_G = 64 (the 4-32-32-9 MLP: 68 fused multiply-adds deep, 2-ulp tanh, feature division), K_T = 8 (3x3 product,
-// subtraction, stored operands), kappa_p because the inverse pivot block is itself computed with roundoff u.
-const double K_G = 64.0, K_T = 8.0;
+// K_G = 128 (the 4-32-32-9 MLP: 68 fused multiply-adds deep with |W| row sums up to ~10, 2-ulp tanh, feature
+// division), K_T = 16 (3x3 product, subtraction, stored operands), kappa_p because the normalised column
+// carries the entry noise of its residual amplified by the inverse pivot block.
+const double K_G = 128.0, K_T = 16.0;
 
 void adj33(const double* A, double* J) {
   J[0] = A[4] * A[8] - A[5] * A[7]; J[1] = A[2] * A[7] - A[1] * A[8]; J[2] = A[1] * A[5] - A[2] * A[4];
@@ -376,7 +380,7 @@ int argmax_score(const std::vector<double>& v, int n, const std::vector<char>& u
 // decisions that are not an arg-max / a correct stop within `slack` (relative).
 void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t snode, double zeta,
                int max_rank, int rule, int rp_rank, const int32_t* rp_i, const int32_t* rp_j,
-               double slack, AcaOut& out, double u_round = 0.0) {
+               double slack, AcaOut& out, double u_round = 0.0, double kappa_max = 300.0, int rp_flag = 0) {
   const Node& T = h.nodes[tnode];
   const Node& S = h.nodes[snode];
   int c = (int)(T.hi - T.lo), q = (int)(S.hi - S.lo);
@@ -384,7 +388,9 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
   const float* Xs = &h.Xs[3 * S.lo];
   int kmax = std::min(std::min(c, q), max_rank);
   bool replay = rp_rank >= 0;
-  if (replay) kmax = std::min(kmax, rp_rank);
+  // a replayed run that broke down (flag 2) lists rp_rank accepted pivots plus the attempted one
+  const int rp_len = replay ? rp_rank + (rp_flag == 2 ? 1 : 0) : 0;
+  if (replay) kmax = std::min(kmax, rp_len);
   std::vector<char> used_r(c, 0), used_c(q, 0);
   std::vector<double> ck((size_t)9 * c), qk((size_t)9 * q);
   std::vector<double> errc(c, 0.0), errq(q, 0.0), kappa;        // replay-mode rounding bounds (checker only)
@@ -433,9 +439,34 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     double P[9], Pinv[9];
     std::memcpy(P, &ck[9 * (size_t)ik], sizeof P);
     double dP = det33(P);
-    if (std::fabs(dP) < 1e-30) { out.flag = 2; break; }         // S-18: singular pivot
+    const bool attempted = replay && rp_flag == 2 && k == rp_rank;       // the step at which the replayed run broke down
+    if (std::fabs(dP) < 1e-30) {                                 // S-18: singular pivot -> breakdown, block goes dense
+      if (replay && !attempted) { out.replay_bad++; out.replay_bad_strict++; }
+      out.flag = 2;
+      out.piv_i.push_back(ik); out.piv_j.push_back(jk);          // the attempted pivot, listed after the rank accepted ones
+      break;
+    }
     inv33(P, dP, Pinv);
     const double kap = std::sqrt(fro2(P) * fro2(Pinv)), pinv_n = std::sqrt(fro2(Pinv));
+    if (!replay && kap > kappa_max) {                            // S-18b: numerically singular pivot
+      out.flag = 2;
+      out.piv_i.push_back(ik); out.piv_j.push_back(jk);
+      break;
+    }
+    // replay: cond_F of the pivot block as the replayed arithmetic can have seen it.  A perturbation of size
+    // e = errc[ik] moves the smallest singular value (~ 1/|P^-1|_F) by up to e.
+    const double e_piv = errc[ik] * pinv_n;
+    const double kap_lo = kap / (1.0 + e_piv), kap_hi = e_piv < 1.0 ? kap / (1.0 - e_piv) : INFINITY;
+    if (attempted) {                                             // replay: the breakdown must be plausible (factor 2 on cond)
+      if (kap < 0.5 * kappa_max) { out.replay_bad_strict++; if (kap_hi < 0.5 * kappa_max) out.replay_bad++; }
+      out.flag = 2;
+      out.piv_i.push_back(ik); out.piv_j.push_back(jk);
+      break;
+    }
+    if (replay && kap > 2.0 * kappa_max) {                       // should have broken down here
+      out.replay_bad_strict++;
+      if (kap_lo > 2.0 * kappa_max) out.replay_bad++;
+    }
     double dc2 = 0;                                             // rounding bound of the normalised column, squared
     // line 6: c_k <- c_k P^{-1}
     for (int i = 0; i < c; ++i) {
@@ -466,7 +497,7 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     double bestc;
     int ruc;
     int jn = argmax_score(qk, q, used_c, rule, &bestc, &ruc);
-    if (replay && k + 1 < rp_rank && jn >= 0) {
+    if (replay && k + 1 < rp_len && jn >= 0) {
       int gj = rp_j[k + 1];
       if (gj < 0 || gj >= q || used_c[gj]) { out.replay_bad++; out.replay_bad_strict++; }
       else {
@@ -528,7 +559,7 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     // line 12: Eq. (10) stop test (S-20)
     bool stop = nu <= zeta * lam;
     if (replay) {
-      bool last = (k + 1 == rp_rank);
+      bool last = (k + 1 == rp_rank) && rp_flag != 2;
       // rounding bound of nu = |c_k q_k^T|_F:  |d nu| <= |dc|_F |q|_F + |c|_F |dq|_F
       double dq2 = 0, cn2 = 0, qn2 = 0;
       for (int j = 0; j < q; ++j) { dq2 += errq[j] * errq[j]; qn2 += fro2(&qk[9 * (size_t)j]); }
@@ -560,6 +591,7 @@ struct Handle {
   Mlp mlp2;
   double a = 1.0;
   double u_round = 0.0;         // replay checker: unit roundoff of the replayed arithmetic (0 = slack only)
+  double kappa_max = 300.0;     // S-18b: pivot blocks with cond_F above this break Alg. 2 down (block goes dense)
   int64_t last_bad_strict = 0;  // slack-only count of the last replay call
 };
 
@@ -715,6 +747,7 @@ void* orc_h_create(int64_t N, const float* X, int leaf, double eta, const int* d
 void orc_h_destroy(void* p) { delete (Handle*)p; }
 // replay checker: unit roundoff of the arithmetic being replayed (2^-24 for the fp32 CUDA path; 0 = slack only)
 void orc_h_set_replay_roundoff(void* p, double u) { ((Handle*)p)->u_round = u; }
+void orc_h_set_kappa_max(void* p, double k) { ((Handle*)p)->kappa_max = k; }
 int64_t orc_h_last_bad_strict(void* p) { return ((Handle*)p)->last_bad_strict; }
 
 void orc_h_counts(void* p, int64_t* n_nodes, int64_t* n_leaves, int64_t* nG, int64_t* nH, int64_t* depth) {
@@ -752,14 +785,15 @@ int orc_h_admissible(void* p, int32_t t, int32_t s) { return admissible(((Handle
 
 // One block of Alg. 2.  C_out [rank][c][9], Q_out [rank][q][9] (capacity cap_rank); returns rank.
 // rp_rank < 0: free run.  rp_rank >= 0: replay with the given pivots (see aca_block).
-int orc_h_aca_block(void* p, int64_t gblock, double zeta, int max_rank, int rule, int rp_rank,
+int orc_h_aca_block(void* p, int64_t gblock, double zeta, int max_rank, int rule, int rp_rank, int rp_flag,
                     const int32_t* rp_i, const int32_t* rp_j, double slack, int cap_rank,
                     double* C_out, double* Q_out, int32_t* piv_i, int32_t* piv_j, double* nu,
                     double* lam, int* flag, int* replay_bad) {
   Handle* H = (Handle*)p;
   auto pr = H->h.G[(size_t)gblock];
   AcaOut o;
-  aca_block(H->h, H->mlp2, H->a, pr.first, pr.second, zeta, max_rank, rule, rp_rank, rp_i, rp_j, slack, o, H->u_round);
+  aca_block(H->h, H->mlp2, H->a, pr.first, pr.second, zeta, max_rank, rule, rp_rank, rp_i, rp_j, slack, o, H->u_round,
+            H->kappa_max, rp_flag);
   H->last_bad_strict = o.replay_bad_strict;
   int c = (int)(H->h.nodes[pr.first].hi - H->h.nodes[pr.first].lo);
   int q = (int)(H->h.nodes[pr.second].hi - H->h.nodes[pr.second].lo);
@@ -771,6 +805,10 @@ int orc_h_aca_block(void* p, int64_t gblock, double zeta, int max_rank, int rule
     if (piv_j) piv_j[k] = o.piv_j[k];
     if (nu) nu[k] = o.nu[k];
     if (lam) lam[k] = o.lam[k];
+  }
+  if (o.flag == 2 && r == o.rank && r < cap_rank && (int)o.piv_i.size() > r) {   // attempted pivot of a breakdown
+    if (piv_i) piv_i[r] = o.piv_i[r];
+    if (piv_j) piv_j[r] = o.piv_j[r];
   }
   if (flag) *flag = o.flag;
   if (replay_bad) *replay_bad = o.replay_bad;
@@ -796,7 +834,7 @@ void orc_h_dense_block(void* p, int64_t gblock, double* G_out) {
 // only_rows: if non-null (tree-order flags, length N) only rows with flag 1 are produced (sampled
 // parity at large N): blocks whose tau range contains no flagged row are skipped.
 int64_t orc_h_matvec(void* p, const float* F, double zeta, int max_rank, int rule, int include_self,
-                     int do_near, int do_far, const int32_t* rp_rank, const int64_t* rp_off,
+                     int do_near, int do_far, const int32_t* rp_rank, const int32_t* rp_flag, const int64_t* rp_off,
                      const int32_t* rp_i, const int32_t* rp_j, double slack,
                      const uint8_t* only_rows, double* U, int32_t* ranks_out, int32_t* flags_out,
                      int64_t* n_entries) {
@@ -845,14 +883,31 @@ int64_t orc_h_matvec(void* p, const float* F, double zeta, int max_rank, int rul
       AcaOut o;
       if (rp_rank)
         aca_block(h, Hd->mlp2, Hd->a, h.G[g].first, h.G[g].second, zeta, max_rank, rule, rp_rank[g],
-                  rp_i + rp_off[g], rp_j + rp_off[g], slack, o, Hd->u_round);
+                  rp_i + rp_off[g], rp_j + rp_off[g], slack, o, Hd->u_round, Hd->kappa_max, rp_flag ? rp_flag[g] : 0);
       else
-        aca_block(h, Hd->mlp2, Hd->a, h.G[g].first, h.G[g].second, zeta, max_rank, rule, -1, nullptr, nullptr, 0.0, o);
+        aca_block(h, Hd->mlp2, Hd->a, h.G[g].first, h.G[g].second, zeta, max_rank, rule, -1, nullptr, nullptr, 0.0, o, 0.0,
+                  Hd->kappa_max, 0);
       entries += (int64_t)o.rank * (c + q);
       bad += o.replay_bad;
       bad_strict += o.replay_bad_strict;
       if (ranks_out) ranks_out[g] = o.rank;
       if (flags_out) flags_out[g] = o.flag;
+      if (o.flag == 2) {                                         // S-18b: Alg. 2 broke down -> the block is applied densely (L252)
+        entries += (int64_t)c * q;
+        for (int64_t i = T.lo; i < T.hi; ++i) {
+          double u[3] = {0, 0, 0};
+          for (int64_t j = S.lo; j < S.hi; ++j) {
+            double M[9];
+            entry2(Hd->mlp2, Hd->a, &h.Xs[3 * i], &h.Xs[3 * j], M);
+            mat3_vec_acc(M, &Fs[3 * j], u);
+          }
+          for (int e = 0; e < 3; ++e) {
+#pragma omp atomic
+            Us[3 * i + e] += u[e];
+          }
+        }
+        continue;
+      }
       for (int k = 0; k < o.rank; ++k) {
         double t[3] = {0, 0, 0};                                 // t = Q_k F^sigma
         for (int j = 0; j < q; ++j) mat3_vec_acc(&o.Q[((size_t)k * q + j) * 9], &Fs[3 * (S.lo + j)], t);

@@ -38,7 +38,8 @@ class _Mlp(C.Structure):
 
 class _Params(C.Structure):
     _fields_ = [("leaf_size", C.c_int32), ("eta", C.c_float), ("aca_tol", C.c_float), ("aca_max_rank", C.c_int32),
-                ("radius_a", C.c_float), ("rcut3", C.c_float), ("pivot_rule", C.c_int32), ("near_path", C.c_int32)]
+                ("radius_a", C.c_float), ("rcut3", C.c_float), ("pivot_rule", C.c_int32), ("near_path", C.c_int32),
+                ("kappa_max", C.c_float)]
 
 
 class Stats(C.Structure):
@@ -47,7 +48,7 @@ class Stats(C.Structure):
                  "far_rows_cols", "sum_rank", "aca_entries", "factor_bytes", "aca_batches", "aca_not_converged",
                  "aca_singular", "n_faces", "workspace_required", "arena_bytes")] + \
                [(n, C.c_float) for n in ("ms_tree", "ms_blocks", "ms_aca", "ms_near", "ms_far", "ms_three", "ms_other", "pad_")] + \
-               [("n_launches", C.c_int64)]
+               [("n_launches", C.c_int64), ("fallback_entries", C.c_int64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -88,7 +89,7 @@ class Context:
     workspace is a torch uint8 CUDA tensor owned here (PyTorch owns all device memory)."""
 
     def __init__(self, mlp2, mlp3=None, leaf_size=64, eta=1.0, aca_tol=1e-4, aca_max_rank=96, radius_a=1.0, rcut3=0.0,
-                 pivot_rule=0, workspace_bytes=None, device="cuda:0", stream=None):
+                 pivot_rule=0, kappa_max=0.0, workspace_bytes=None, device="cuda:0", stream=None):
         import torch
         self.torch = torch
         self.lib = load()
@@ -102,7 +103,7 @@ class Context:
         self.workspace = torch.empty(int(workspace_bytes) // 256 * 256, dtype=torch.uint8, device=self.device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._keep = []
-        self.params = _Params(leaf_size, eta, aca_tol, aca_max_rank, radius_a, rcut3, pivot_rule, 0)
+        self.params = _Params(leaf_size, eta, aca_tol, aca_max_rank, radius_a, rcut3, pivot_rule, 0, kappa_max)
         m2 = self._mlp_struct(mlp2)
         m3 = self._mlp_struct(mlp3) if mlp3 is not None else None
         self._h = C.c_void_p()
@@ -228,7 +229,8 @@ class Context:
         self._chk(self.lib.hh_get_factors(self._h, C.c_int64(block), C.byref(rank), C.byref(flag), C.c_int32(cap_rank),
                                           _ptr(pi), _ptr(pj), _ptr(Cf), _ptr(Qf)))
         r = rank.value
-        return dict(rank=r, flag=flag.value, piv_i=pi[:r], piv_j=pj[:r], C=None if Cf is None else Cf[:r],
+        npiv = min(cap_rank, r + (1 if flag.value == 2 else 0))      # a breakdown also lists its attempted pivot
+        return dict(rank=r, flag=flag.value, piv_i=pi[:npiv], piv_j=pj[:npiv], C=None if Cf is None else Cf[:r],
                     Q=None if Qf is None else Qf[:r])
 
     def eval_entries(self, Xi, Xj):

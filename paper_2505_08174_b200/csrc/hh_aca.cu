@@ -12,7 +12,7 @@
 #include "hh_mlp.cuh"
 
 struct AcaArgs {
-  const float* w2; float a; float tol; int max_rank; int rule;
+  const float* w2; float a; float tol; int max_rank; int rule; double kappa_max;
   const uint2* PG; const u32 *nlo, *nhi; const float* Xs;
   float* arena; u64 arena_units; u32* tab; DevScalars* sc;
   int *ranks, *flags;
@@ -190,11 +190,15 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 384 / T) k_aca(AcaArgs A) {
         S.sPinvD[4] = (P[0] * P[8] - P[2] * P[6]) * iv; S.sPinvD[5] = (P[2] * P[3] - P[0] * P[5]) * iv;
         S.sPinvD[6] = (P[3] * P[7] - P[4] * P[6]) * iv; S.sPinvD[7] = (P[1] * P[6] - P[0] * P[7]) * iv;
         S.sPinvD[8] = (P[0] * P[4] - P[1] * P[3]) * iv;
+        double np2 = 0.0, ni2 = 0.0;
+#pragma unroll
+        for (int r = 0; r < 9; ++r) { np2 += P[r] * P[r]; ni2 += S.sPinvD[r] * S.sPinvD[r]; }
+        if (sqrt(np2 * ni2) > A.kappa_max) S.ctl[1] = 2;          // S-18b: numerically singular at fp32 entry accuracy
       }
       S.piv_i[k] = ik;
     }
     __syncthreads();
-    if (S.ctl[1] == 2) { flag = 2; break; }                     // S-18: singular pivot -> stop at the current rank
+    if (S.ctl[1] == 2) { flag = 2; break; }                     // S-18 / S-18b: breakdown -> the block is applied densely
 
     // ---- line 6: c_k(i) = c'_k(i) P^{-1} (fp64 products, rounded once); Gram matrices A_kk, A_pk (S-19) ----
     {
@@ -342,7 +346,8 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 384 / T) k_aca(AcaArgs A) {
   if (tid == 0) { A.ranks[g] = rank; A.flags[g] = flag; }
   for (int t = tid; t < HH_MAX_CHUNKS; t += T) tabrow[t] = (t * HH_RC < rank) ? S.chunk[t] : 0xffffffffu;
   int* piv = (int*)(A.arena + (size_t)tabrow[HH_TAB_PIV] * HH_UNIT_FLOATS);
-  for (int t = tid; t < rank; t += T) { piv[t] = S.piv_i[t]; piv[HH_MAX_RANK + t] = S.piv_j[t]; }
+  // a breakdown (flag 2) also lists the attempted pivot after the accepted ones
+  for (int t = tid; t < rank + (flag == 2 ? 1 : 0); t += T) { piv[t] = S.piv_i[t]; piv[HH_MAX_RANK + t] = S.piv_j[t]; }
 }
 
 // ------------------------------------------------------------------------------ batching (L246, L260)
@@ -361,13 +366,16 @@ __global__ void k_batch_range(const u64* __restrict__ unit_prefix, u32 first, u3
   sc->fail_min = 0xffffffffu;
   sc->sum_rank = sc->aca_entries = sc->factor_bytes = 0;
   sc->not_conv = sc->singular = sc->max_rank_seen = 0;
+  sc->n_dense = 0;
+  sc->fallback_entries = 0;
 }
 
 __global__ void __launch_bounds__(256) k_batch_stats(const uint2* __restrict__ PG, const u32* __restrict__ nlo,
                                                       const u32* __restrict__ nhi, int* __restrict__ ranks,
-                                                      const int* __restrict__ flags, u32 first, u32 next, u32 end, DevScalars* sc) {
+                                                      const int* __restrict__ flags, u32 first, u32 next, u32 end,
+                                                      u32* __restrict__ dense_list, DevScalars* sc) {
   u32 g = first + blockIdx.x * blockDim.x + threadIdx.x;
-  u64 sr = 0, en = 0;
+  u64 sr = 0, en = 0, fu = 0;
   u32 nc = 0, sg = 0, mr = 0;
   if (g < next) {
     uint2 p = PG[g];
@@ -375,17 +383,24 @@ __global__ void __launch_bounds__(256) k_batch_stats(const uint2* __restrict__ P
     int r = ranks[g];
     sr = (u64)r; en = (u64)r * mn; mr = (u32)r;
     nc = flags[g] == 1; sg = flags[g] == 2;
+    fu = sg ? 0 : en;                                            // factor entries the far-field apply reads
+    if (sg) {                                                    // S-18b: applied densely by hh_dense_apply
+      dense_list[atomicAdd(&sc->n_dense, 1u)] = g;
+      atomicAdd((unsigned long long*)&sc->fallback_entries, (unsigned long long)(nhi[p.x] - nlo[p.x]) * (nhi[p.y] - nlo[p.y]));
+    }
   } else if (g < end) {
     ranks[g] = -1;                                               // factorised past the failure point: discarded
   }
   for (int o = 16; o; o >>= 1) {
     sr += __shfl_xor_sync(0xffffffffu, sr, o); en += __shfl_xor_sync(0xffffffffu, en, o);
+    fu += __shfl_xor_sync(0xffffffffu, fu, o);
     nc += __shfl_xor_sync(0xffffffffu, nc, o); sg += __shfl_xor_sync(0xffffffffu, sg, o);
     mr = max(mr, __shfl_xor_sync(0xffffffffu, mr, o));
   }
   if ((threadIdx.x & 31) == 0) {
     atomicAdd((unsigned long long*)&sc->sum_rank, (unsigned long long)sr);
     atomicAdd((unsigned long long*)&sc->aca_entries, (unsigned long long)en);
+    atomicAdd((unsigned long long*)&sc->factor_bytes, (unsigned long long)fu * 36ull);
     atomicAdd(&sc->not_conv, nc); atomicAdd(&sc->singular, sg); atomicMax(&sc->max_rank_seen, mr);
   }
 }
@@ -411,6 +426,7 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   ctx->arena_units = (ctx->scratch_bytes - tab_bytes) / 128;
   AcaArgs A;
   A.w2 = ctx->w2; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.max_rank = ctx->p.aca_max_rank; A.rule = ctx->p.pivot_rule;
+  A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : 300.0;
   A.PG = ctx->PG; A.nlo = ctx->nlo; A.nhi = ctx->nhi; A.Xs = ctx->Xs;
   A.arena = ctx->arena; A.arena_units = ctx->arena_units; A.tab = ctx->tab; A.sc = ctx->d_sc;
   A.ranks = ctx->ranks; A.flags = ctx->flags; A.first = (u32)first;
@@ -430,7 +446,8 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->fail_min, &ctx->d_sc->fail_min, sizeof(u32), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   u32 nx = ctx->h_sc->fail_min < end ? ctx->h_sc->fail_min : end;
-  k_batch_stats<<<HH_N + cdiv(nb, 256), 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, (u32)first, nx, end, ctx->d_sc);
+  k_batch_stats<<<HH_N + cdiv(nb, 256), 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, (u32)first, nx, end,
+                                                             ctx->dense_list, ctx->d_sc);
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   const DevScalars& h = *ctx->h_sc;
@@ -440,9 +457,11 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   if (nx <= first) return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "factor arena cannot hold a single admissible block");
   ctx->st.sum_rank += (int64_t)h.sum_rank;
   ctx->st.aca_entries += (int64_t)h.aca_entries;
-  ctx->st.factor_bytes += (int64_t)h.aca_entries * 36;
+  ctx->st.factor_bytes += (int64_t)h.factor_bytes;
   ctx->st.aca_not_converged += h.not_conv;
   ctx->st.aca_singular += h.singular;
+  ctx->st.fallback_entries += (int64_t)h.fallback_entries;
+  ctx->n_dense = h.n_dense;
   ctx->st.aca_batches += 1;
   // next prediction: what this batch really used per predicted chunk, plus 10 %
   if (nx > first) {
@@ -478,10 +497,13 @@ int hh_factors_fetch(hh_ctx* ctx, int64_t block, int32_t* rank, int32_t* flag, i
   if (flag) *flag = f;
   if (r < 0) return hh_fail(ctx, HH_ERR_INVALID_ARG, "block has not been factorised");
   int rr = r < cap_rank ? r : cap_rank;
-  if ((piv_i || piv_j) && rr > 0) {
+  int np_ = r + (f == 2 ? 1 : 0);                                // a breakdown also lists its attempted pivot
+  if (np_ > cap_rank) np_ = cap_rank;
+  if (np_ > HH_MAX_RANK) np_ = HH_MAX_RANK;
+  if ((piv_i || piv_j) && np_ > 0) {
     int piv[2 * HH_MAX_RANK];
     HH_CUDA(cudaMemcpy(piv, ctx->arena + (size_t)row[HH_TAB_PIV] * HH_UNIT_FLOATS, sizeof piv, cudaMemcpyDeviceToHost));
-    for (int k = 0; k < rr; ++k) { if (piv_i) piv_i[k] = piv[k]; if (piv_j) piv_j[k] = piv[HH_MAX_RANK + k]; }
+    for (int k = 0; k < np_; ++k) { if (piv_i) piv_i[k] = piv[k]; if (piv_j) piv_j[k] = piv[HH_MAX_RANK + k]; }
   }
   if (C || Q) {
     float* tmp = (float*)malloc(sizeof(float) * 9 * (size_t)(mp > np ? mp : np));

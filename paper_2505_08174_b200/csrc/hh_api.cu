@@ -42,6 +42,7 @@ static int carve(hh_ctx* ctx, int64_t N) {
   ctx->near_begin = c.take<u32>(nodes); ctx->near_end = c.take<u32>(nodes);
   ctx->PG = c.take<uint2>(ctx->cap_pairs); ctx->PH = c.take<uint2>(ctx->cap_pairs);
   ctx->ranks = c.take<int>(ctx->cap_pairs); ctx->flags = c.take<int>(ctx->cap_pairs);
+  ctx->dense_list = c.take<u32>(ctx->cap_pairs);
   ctx->unit_prefix = c.take<u64>(ctx->cap_pairs + 1);
   ctx->n_cells_cap = 4 * N + 4096;
   ctx->cell_of = c.take<u32>(N); ctx->cell_order = c.take<u32>(N); ctx->cell_start = c.take<u32>(ctx->n_cells_cap + 1);
@@ -69,6 +70,7 @@ static int check_params(const hh_params* p) {
   if (!(p->rcut3 >= 0.f) || !isfinite(p->rcut3)) return 0;
   if (p->pivot_rule != 0 && p->pivot_rule != 1) return 0;
   if (p->near_path != 0) return 0;
+  if (!(p->kappa_max >= 0.f)) return 0;                           /* 0 = default, INFINITY allowed, NaN / negative not */
   return 1;
 }
 
@@ -181,7 +183,8 @@ extern "C" int hh_set_params(hh_ctx* ctx, const hh_params* params) {
   if (params->rcut3 > 0.f && !ctx->have_mlp3) return hh_fail(ctx, HH_ERR_INVALID_ARG, "rcut3 > 0 needs a three-body MLP");
   if (params->leaf_size != ctx->p.leaf_size) ctx->tree_ok = ctx->blocks_ok = 0;
   if (params->eta != ctx->p.eta) ctx->blocks_ok = 0;
-  ctx->res_first = ctx->res_next = 0;               // factors depend on tol / rank cap / rule
+  ctx->res_first = ctx->res_next = 0;               // factors depend on tol / rank cap / rule / kappa_max
+  ctx->n_dense = 0;
   ctx->l_pred = 32.0;
   ctx->p = *params;
   return HH_OK;
@@ -270,10 +273,14 @@ extern "C" int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts)
       HH_TRY(hh_far_apply(ctx));
       T0(5);
       if (ctx->timing) ctx->st.ms_far += ev_ms(ctx, 4, 5);
+      T0(4);
+      HH_TRY(hh_dense_apply(ctx));
+      T0(5);
+      if (ctx->timing) ctx->st.ms_near += ev_ms(ctx, 4, 5);
     } else {
       // factors are streamed through the arena batch by batch (L246, L260, L334)
       ctx->st.sum_rank = ctx->st.aca_entries = ctx->st.factor_bytes = ctx->st.aca_batches = 0;
-      ctx->st.aca_not_converged = ctx->st.aca_singular = 0;
+      ctx->st.aca_not_converged = ctx->st.aca_singular = ctx->st.fallback_entries = 0;
       int64_t first = 0;
       while (first < ctx->nG) {
         int64_t next = first;
@@ -283,6 +290,10 @@ extern "C" int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts)
         HH_TRY(hh_far_apply(ctx));
         T0(5);
         if (ctx->timing) ctx->st.ms_far += ev_ms(ctx, 4, 5);
+        T0(4);
+        HH_TRY(hh_dense_apply(ctx));
+        T0(5);
+        if (ctx->timing) ctx->st.ms_near += ev_ms(ctx, 4, 5);
         first = next;
       }
     }
@@ -313,6 +324,7 @@ extern "C" int hh_far_apply_resident(hh_ctx* ctx, const float* F, float* U) {
   HH_TRY(hh_far_apply(ctx));
   T0(5);
   if (ctx->timing) ctx->st.ms_far = ev_ms(ctx, 4, 5);
+  HH_TRY(hh_dense_apply(ctx));
   k_unpermute<<<HH_N + cdiv(N, 256), 256, 0, ctx->stream>>>(ctx->Us, ctx->Fs, ctx->perm, N, 0, 0, U);
   HH_LAUNCH_CHECK();
   return HH_OK;

@@ -21,7 +21,7 @@ __device__ __forceinline__ float ldg_stream1(const float* p) {
 // T threads; JT = source columns staged per tile (>= the largest n of the size class, or 2048 with tiling)
 template <int T, int JT>
 __global__ void __launch_bounds__(T) k_far(const uint2* __restrict__ PG, const u32* __restrict__ nlo, const u32* __restrict__ nhi,
-                                            const int* __restrict__ ranks, const u32* __restrict__ tab, const float* __restrict__ arena,
+                                            const int* __restrict__ ranks, const int* __restrict__ flags, const u32* __restrict__ tab, const float* __restrict__ arena,
                                             const float* __restrict__ Fs, float* __restrict__ Us, u32 first, u32 begin) {
   __shared__ __align__(16) float sF[3][JT];        // component-major force tile
   __shared__ float st[HH_MAX_RANK * 3];                // t_k = Q_k F^sigma
@@ -30,7 +30,7 @@ __global__ void __launch_bounds__(T) k_far(const uint2* __restrict__ PG, const u
   constexpr int NW = T / 32;
   const u32 g = begin + blockIdx.x;
   const int l = ranks[g];
-  if (l <= 0) return;
+  if (l <= 0 || flags[g] == 2) return;             // nothing factorised / Alg. 2 broke down (applied densely, S-18b)
   const uint2 blk = PG[g];
   const u32 tlo = nlo[blk.x], m = nhi[blk.x] - tlo;
   const u32 slo = nlo[blk.y], n = nhi[blk.y] - slo;
@@ -101,10 +101,10 @@ int hh_far_apply(hh_ctx* ctx) {
     u32 e = ctx->class_bound[c + 1] < end ? ctx->class_bound[c + 1] : end;
     if (b >= e) continue;
     switch (c) {
-      case 0: k_far<512, 2048><<<HH_N + e - b, 512, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      case 1: k_far<256, 256><<<HH_N + e - b, 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      case 2: k_far<128, 128><<<HH_N + e - b, 128, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      default: k_far<64, 64><<<HH_N + e - b, 64, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 0: k_far<512, 2048><<<HH_N + e - b, 512, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 1: k_far<256, 256><<<HH_N + e - b, 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 2: k_far<128, 128><<<HH_N + e - b, 128, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      default: k_far<64, 64><<<HH_N + e - b, 64, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
     }
   }
   HH_LAUNCH_CHECK();

@@ -46,7 +46,8 @@ struct DevScalars {
   u64 sum_rank, aca_entries, factor_bytes, n_faces;
   u32 not_conv, singular, deg_overflow, pad1;
   u64 near_entries, far_rows_cols;
-  u32 max_rank_seen, pad2;
+  u32 max_rank_seen, n_dense;
+  u64 fallback_entries;
 };
 
 struct hh_ctx {
@@ -85,6 +86,7 @@ struct hh_ctx {
   uint2 *PG, *PH;                       /* (tau, sigma) node ids; PG sorted by size desc, PH by tau */
   u32 *near_begin, *near_end;           /* per node: range in PH                              */
   int* ranks; int* flags;               /* per admissible block                               */
+  u32* dense_list; u32 n_dense;         /* resident blocks on which Alg. 2 broke down (S-18b): applied densely */
   u64* unit_prefix;                     /* prefix of (m_pad + n_pad) over sorted PG, nG+1     */
   char* scratch; size_t scratch_bytes;  /* frontier ping-pong during build; == arena region    */
   float* arena; u64 arena_units;        /* after the resident table                            */
@@ -126,6 +128,7 @@ int hh_sort_pairs(hh_ctx* ctx, u64* keys[2], u32* vals[2], int64_t n, int bit_lo
 int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N);
 int hh_blocks_build(hh_ctx* ctx);
 int hh_near_apply(hh_ctx* ctx);                                       /* Us += near-field           */
+int hh_dense_apply(hh_ctx* ctx);                                      /* Us += resident blocks on which ACA broke down, densely */
 int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next);
 int hh_far_apply(hh_ctx* ctx);                                        /* Us += resident far-field   */
 int hh_three_apply(hh_ctx* ctx);                                     /* Us += three-body term (tree order) */

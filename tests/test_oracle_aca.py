@@ -25,7 +25,9 @@ def flat(G):
 @pytest.fixture(scope="module")
 def H_small(mlp2):
     X = synth.cube_cloud(1200, 0.1, seed=30)
-    return oracle.HMatrix(X, mlp2, leaf=16, eta=1.0)
+    H = oracle.HMatrix(X, mlp2, leaf=16, eta=1.0)
+    H.set_kappa_max(float("inf"))          # these pins are about the plain listing (no S-18b breakdown)
+    return H
 
 
 def big_blocks(H, k=4):
@@ -200,6 +202,7 @@ def test_matvec_pieces_add_up_and_caller_order(mlp2):
     X = synth.cube_cloud(900, 0.1, seed=36)
     F = synth.gaussian_forces(900, seed=37)
     H = oracle.HMatrix(X, mlp2, leaf=16, eta=1.0)
+    H.set_kappa_max(float("inf"))          # plain listing; S-18b has its own test below
     U, _ = H.matvec(F, 1e-4)
     Un, _ = H.matvec(F, 1e-4, include_self=False, far=False)
     Uf, _ = H.matvec(F, 1e-4, include_self=False, near=False)
@@ -207,6 +210,7 @@ def test_matvec_pieces_add_up_and_caller_order(mlp2):
     # permuting the caller's particle order permutes U (tree order is internal, S-9)
     p = np.random.default_rng(1).permutation(900)
     Hp = oracle.HMatrix(X[p], mlp2, leaf=16, eta=1.0)
+    Hp.set_kappa_max(float("inf"))
     Up, _ = Hp.matvec(F[p], 1e-4)
     assert rel_l2(Up, U[p]) < 1e-12
     # sampled rows agree with the full product
@@ -224,3 +228,52 @@ def test_matvec_pieces_add_up_and_caller_order(mlp2):
         ranks.append(r["rank"]); piv_i.append(r["piv_i"]); piv_j.append(r["piv_j"])
     Ur, info = H.matvec(F, 1e-4, replay=(np.array(ranks), np.concatenate(piv_i), np.concatenate(piv_j)))
     assert info["replay_bad"] == 0 and rel_l2(Ur, U) < 1e-14      # (OpenMP sum order)
+
+
+def test_breakdown_on_ill_conditioned_pivot_goes_dense(mlp2):
+    """S-18b: a pivot block with cond_F > kappa_max breaks Alg. 2 down; the block is flagged and the mat-vec
+    evaluates it densely, which is exact (L252, L283).  Bead chains (collinear points) produce such pivots."""
+    X = synth.chain_cloud(40, 50, 0.1)
+    F = synth.gaussian_forces(len(X))
+    H = oracle.HMatrix(X, mlp2, leaf=16, eta=1.0)
+    Ud = oracle.dense_matvec(X, F, mlp2)
+    U300, i300 = H.matvec(F, 1e-4)
+    flagged = np.flatnonzero(i300["flags"] == 2)
+    assert len(flagged) > 0 and len(flagged) < 0.2 * H.nG
+    # every flagged block really has an ill-conditioned pivot at the step after its last accepted one
+    H.set_kappa_max(float("inf"))
+    for g in flagged[:20]:
+        r = H.aca_block(int(g), 1e-4)
+        k = i300["ranks"][g]
+        if r["flag"] == 2 and r["rank"] == k:
+            continue                          # exactly singular pivot (S-18): no factor row to look at
+        assert r["rank"] > k
+        P = r["Q"][k][r["piv_j"][k]]
+        assert np.linalg.norm(P) * np.linalg.norm(np.linalg.inv(P)) > 300.0
+        for kk in range(k):
+            Pk = r["Q"][kk][r["piv_j"][kk]]
+            assert np.linalg.norm(Pk) * np.linalg.norm(np.linalg.inv(Pk)) <= 300.0
+    Uinf, iinf = H.matvec(F, 1e-4)
+    # without S-18b only exactly singular pivots (|det| < 1e-30, S-18) break down
+    assert set(np.flatnonzero(iinf["flags"] == 2)) < set(flagged)
+    # both within the tolerance of the dense product; dense entries are counted in place of the rank terms
+    assert rel_l2(U300, Ud) <= 1e-4 and rel_l2(Uinf, Ud) <= 1e-4
+    shapes = np.array([H.block_shape(int(g)) for g in range(H.nG)])
+    expect = int(np.sum(i300["ranks"] * shapes.sum(1)) + np.sum((i300["flags"] == 2) * shapes[:, 0] * shapes[:, 1]))
+    near = sum(int((H.hi[t] - H.lo[t]) * (H.hi[s] - H.lo[s])) for t, s in H.H) - H.N
+    assert i300["entries"] == expect + near
+    # replaying a run with its own pivots and flags is the identity, and an implausible breakdown is reported
+    H.set_kappa_max(300.0)
+    ranks, flags = i300["ranks"], i300["flags"]
+    pi, pj = [], []
+    for g in range(H.nG):
+        r = H.aca_block(g, 1e-4)
+        assert r["rank"] == ranks[g] and r["flag"] == flags[g] and len(r["piv_i"]) == ranks[g] + (flags[g] == 2)
+        pi.append(r["piv_i"]); pj.append(r["piv_j"])
+    Ur, ir = H.matvec(F, 1e-4, replay=(ranks, np.concatenate(pi), np.concatenate(pj), flags))
+    assert ir["replay_bad"] == 0 and rel_l2(Ur, U300) < 1e-13 and np.array_equal(ir["flags"], flags)
+    g = int(np.flatnonzero(flags == 0)[0])
+    r = H.aca_block(g, 1e-4)
+    assert r["rank"] >= 2
+    bogus = H.aca_block(g, 1e-4, replay=(r["piv_i"][:2], r["piv_j"][:2]), replay_flag=2)
+    assert bogus["flag"] == 2 and bogus["replay_bad"] > 0

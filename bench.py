@@ -284,7 +284,7 @@ def run_gpu(args):
         "apply_only": {"value": N / (apply_ms * 1e-3) if apply_ms > 0 else None, "unit": UNIT,
                        "what": "near + far + three-body + self/permute with factors given (ACA, tree, blocks excluded)"},
         "counts": {k: st[k] for k in ("n_nodes", "n_leaves", "n_admissible", "n_inadmissible", "near_entries", "far_rows_cols",
-                                      "sum_rank", "aca_entries", "factor_bytes", "aca_not_converged", "aca_singular", "n_faces")},
+                                      "sum_rank", "aca_entries", "factor_bytes", "aca_not_converged", "aca_singular", "fallback_entries", "n_faces")},
         "roofline": {"kernel": "k_far (far-field apply U^tau += C (Q F^sigma), all size classes and arena batches of one step)",
                      "bound": "hbm", "achieved": far_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": far_gbs / hbm_peak,
                      "traffic": None, "peak_source": peak_src, "share_of_step": far_ms / step_ms,

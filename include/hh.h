@@ -109,6 +109,10 @@ int hh_destroy(hh_ctx* ctx);
  * sweeps of config 3).  Invalidates tree and blocks as needed. */
 int hh_set_params(hh_ctx* ctx, const hh_params* params);
 
+/* Alg. 2 form: 0 = lock-step over all blocks of an arena batch (default), 1 = one CTA per block.
+ * Same factors up to fp32 summation order in the norm recursion. */
+int hh_set_aca_impl(hh_ctx* ctx, int impl);
+
 /* Record per-stage CUDA-event times into hh_stats (adds stream synchronisations). */
 int hh_enable_timing(hh_ctx* ctx, int on);
 

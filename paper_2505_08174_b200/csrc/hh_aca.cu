@@ -443,6 +443,13 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     }
   }
   HH_LAUNCH_CHECK();
+  return hh_aca_batch_finish(ctx, first, end, next);
+}
+
+// shared by both ACA forms: batch boundary, counters, dense list (S-18b), rank prediction for the next batch
+int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next) {
+  cudaStream_t s = ctx->stream;
+  const u32 nb = end - (u32)first;
   HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->fail_min, &ctx->d_sc->fail_min, sizeof(u32), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   u32 nx = ctx->h_sc->fail_min < end ? ctx->h_sc->fail_min : end;

@@ -1,0 +1,510 @@
+// hh_aca2.cu -- SURVEY 8(a) row 7, lock-step form: Alg. 2 (Eqs. (8)-(10)) run on ALL admissible
+// blocks of an arena batch at once, one listing line per kernel, the way the paper's own implementation does it
+// (L262: "lines 2-12 each a parallel_for over the selected blocks; lines 4, 7 = gather coords -> NN inference ->
+// scatter into C / Q") -- done the B200 way: no coordinate matrices Y, Z and no separate inference call; the rows
+// (line 4) resp. columns (line 7) of all active blocks are cut into 16-entry granules, the granules of one
+// iteration form one flat, load-balanced work list, and the MLP is evaluated in registers exactly as in the
+// near-field kernel (hh_mlp.cuh).  A 2^19-row top-level block and a 20-row leaf block cost the same per entry.
+//
+// One iteration k (all blocks in lock step; blocks drop out as they stop):
+//   k_col   line 4-5  c'(i) = G(i,j_k) - sum_p C_p(i) Q_p(j_k), stored raw; arg-max scores (Eq. (9), S-18) by atomicMax
+//   k_piv   line 5-6  pivot row i_k, P = c'(i_k), P^-1 and cond_F(P) in fp64; zero column -> done (S-21); singular or
+//                     cond_F > kappa_max -> breakdown, block goes dense (S-18, S-18b)
+//   k_norm  line 6    c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk, A_pk = sum_i C_p(i)^T c_k(i)   (S-19)
+//   k_row   line 7-8  q_k(j) = G(i_k,j) - sum_p C_p(i_k) Q_p(j), stored raw; arg-max for j_{k+1}; B_kk, B_kp = sum_j q_k(j) Q_p(j)^T
+//   k_fin   line 9-12 nu^2 = tr(A_kk B_kk), lambda^2 += nu^2 + 2 sum_p tr(A_pk B_kp); stop test Eq. (10) (S-20);
+//                     next column; arena space for the next HH_RC ranks
+// Storage, arena chunks, table rows and the pivot record are those of hh_aca.cu (the far-field kernel reads both).
+#include "hh_mlp.cuh"
+
+#define GR 16                    /* entries per granule = half a warp                                   */
+#define A2_T 256                 /* threads of the entry-evaluating kernels                              */
+
+struct BlkState {                /* 64 bytes per block of the batch                                      */
+  u32 tlo, slo, m, n;
+  int k;                         /* step = number of accepted rank terms                                 */
+  int jk, ik;                    /* current column / pivot row                                           */
+  int status;                    /* 0 active, 1 done, 2 breakdown (dense), -1 arena space failed         */
+  float lam2;
+  int flag;
+  int kmax;
+  u32 pad[5];
+};
+
+struct A2Args {
+  const float* w2; float a; float tol; int rule; double kappa_max;
+  const uint2* PG; const u32 *nlo, *nhi; const float* Xs;
+  float* arena; u64 arena_units; u32* tab; DevScalars* sc;
+  int *ranks, *flags;
+  u32 first, nb;
+  int R;                         /* rank cap of the context: accumulators hold R + 1 Gram slots          */
+  BlkState* st; unsigned long long* amax; double* pinv; float* acc;
+  u32 *cm, *cn; uint2 *gm, *gn;
+};
+
+__device__ __forceinline__ u32 a2_pad8(u32 v) { return (v + 7u) & ~7u; }
+__device__ __forceinline__ int acc_stride(int R) { return 18 + 18 * (R + 1); }
+/* accumulators of a block: [0,9) A_kk, [9,18) B_kk, 18 + 9p: A_pk, 18 + 9(R+1) + 9p: B_kp                 */
+__device__ __forceinline__ float* chunk_ptr(const A2Args& A, const u32* tabrow, int p) {
+  return A.arena + (size_t)tabrow[p / HH_RC] * HH_UNIT_FLOATS;
+}
+__device__ __forceinline__ unsigned long long amax_key(float score, u32 idx) {   // larger score wins, ties -> lowest index
+  return ((unsigned long long)__float_as_uint(score) << 32) | (unsigned long long)(0xffffffffu - idx);
+}
+__device__ __forceinline__ float half_sum(float v) {                             // sum over the 16 lanes of a half-warp
+#pragma unroll
+  for (int o = 8; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ unsigned long long half_max(unsigned long long v) {
+#pragma unroll
+  for (int o = 8; o; o >>= 1) { unsigned long long t = __shfl_xor_sync(0xffffffffu, v, o); v = t > v ? t : v; }
+  return v;
+}
+
+// ---- arena space for ranks k .. k+HH_RC-1 of one block (plus the pivot record with the first chunk) ----
+__device__ __forceinline__ bool a2_alloc(const A2Args& A, u32 b, const BlkState& s, int k) {
+  const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
+  const u32 chunk_units = 9u * (mp + np) / 8u;
+  u32* tabrow = A.tab + (size_t)b * HH_TAB_STRIDE;
+  const u32 need = chunk_units + (k == 0 ? 6u : 0u);
+  u64 off = atomicAdd((unsigned long long*)&A.sc->arena_cursor, (unsigned long long)need);
+  if (off + need > A.arena_units) { atomicMin(&A.sc->fail_min, A.first + b); return false; }
+  if (k == 0) { tabrow[HH_TAB_PIV] = (u32)off; off += 6; }
+  tabrow[k / HH_RC] = (u32)off;
+  return true;
+}
+__device__ __forceinline__ int* a2_piv(const A2Args& A, u32 b) {
+  return (int*)(A.arena + (size_t)A.tab[(size_t)b * HH_TAB_STRIDE + HH_TAB_PIV] * HH_UNIT_FLOATS);
+}
+__device__ __forceinline__ void a2_zero_acc(const A2Args& A, u32 b, int k) {      // slots used by step k
+  float* acc = A.acc + (size_t)b * acc_stride(A.R);
+  for (int t = 0; t < 18; ++t) acc[t] = 0.f;
+  for (int t = 0; t < 9 * k; ++t) { acc[18 + t] = 0.f; acc[18 + 9 * (A.R + 1) + t] = 0.f; }
+  for (int t = 0; t < 4; ++t) A.amax[(size_t)b * 4 + t] = 0ull;
+}
+__device__ __forceinline__ void a2_finish(const A2Args& A, u32 b, BlkState& s, int status, int flag) {
+  s.status = status; s.flag = flag;
+  A.ranks[A.first + b] = s.k;
+  A.flags[A.first + b] = flag;
+  u32* tabrow = A.tab + (size_t)b * HH_TAB_STRIDE;
+  for (int t = (s.k + HH_RC - 1) / HH_RC; t < HH_MAX_CHUNKS; ++t) tabrow[t] = 0xffffffffu;
+}
+
+__global__ void __launch_bounds__(256) k2_init(A2Args A) {
+  const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= A.nb) return;
+  const uint2 blk = A.PG[A.first + b];
+  BlkState s;
+  s.tlo = A.nlo[blk.x]; s.m = A.nhi[blk.x] - s.tlo;
+  s.slo = A.nlo[blk.y]; s.n = A.nhi[blk.y] - s.slo;
+  s.k = 0; s.jk = 0; s.ik = -1;                                   // S-17: j_1 = 0
+  s.lam2 = 0.f; s.flag = 0; s.status = 0;
+  s.kmax = min(min((int)s.m, (int)s.n), A.R);
+  for (int t = 0; t < 5; ++t) s.pad[t] = 0;
+  A.ranks[A.first + b] = -1; A.flags[A.first + b] = 0;
+  if (!a2_alloc(A, b, s, 0)) s.status = -1;
+  else { a2_piv(A, b)[HH_MAX_RANK] = 0; a2_zero_acc(A, b, 0); }
+  A.st[b] = s;
+}
+
+// ---- granule lists of the iteration: one (block, first entry) pair per 16 rows resp. columns of every active block ----
+__global__ void __launch_bounds__(256) k2_gran_count(A2Args A) {
+  const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
+  u32 act = 0;
+  if (b < A.nb) {
+    const BlkState& s = A.st[b];
+    act = s.status == 0;
+    A.cm[b] = act ? (s.m + GR - 1) / GR : 0u;
+    A.cn[b] = act ? (s.n + GR - 1) / GR : 0u;
+  }
+  act = __popc(__ballot_sync(0xffffffffu, act));
+  if ((threadIdx.x & 31) == 0 && act) atomicAdd(&A.sc->n_split, act);        // n_split doubles as the active-block count here
+}
+__global__ void __launch_bounds__(256) k2_gran_fill(A2Args A) {                // one warp per block
+  const u32 b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+  if (b >= A.nb) return;
+  const BlkState& s = A.st[b];
+  if (s.status != 0) return;
+  const u32 nm = (s.m + GR - 1) / GR, nn = (s.n + GR - 1) / GR, pm = A.cm[b], pn = A.cn[b];
+  for (u32 t = lane; t < nm; t += 32) A.gm[pm + t] = make_uint2(b, t * GR);
+  for (u32 t = lane; t < nn; t += 32) A.gn[pn + t] = make_uint2(b, t * GR);
+}
+
+// ---- lines 4-5 (COLS = false: over the rows of tau) and lines 7-8 (COLS = true: over the columns of sigma) ----
+// A warp takes 4 granules: slot (e, half) -> granule 4*tile + 2*e + half; every thread evaluates two entries.
+template <bool COLS>
+__global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
+  __shared__ __align__(16) float sw[HH_MLP2_FLOATS];
+  load_weights(sw, A.w2, HH_MLP2_FLOATS);
+  __syncthreads();
+  const u32 lane = threadIdx.x & 31, half = lane >> 4, l16 = lane & 15, warp = threadIdx.x >> 5;
+  const uint2* gl = COLS ? A.gn : A.gm;
+  const u32 ntiles = (count + 3) / 4;
+  for (u32 tile = blockIdx.x * (A2_T / 32) + warp; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
+    u32 bb[2], idx[2], len[2], lenp[2];
+    int kk[2];
+    bool ok[2];
+    float xi[2][3], xj[2][3], v[2][9];
+    const u32* tabrow[2];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const u32 gi = 4 * tile + 2 * e + half;
+      const bool gv = gi < count;
+      const uint2 g = gl[gv ? gi : count - 1];
+      bb[e] = g.x; idx[e] = g.y + l16;
+      const BlkState& s = A.st[g.x];
+      len[e] = COLS ? s.n : s.m;
+      lenp[e] = a2_pad8(len[e]);
+      kk[e] = s.k;
+      ok[e] = gv && s.status == 0 && idx[e] < len[e];
+      tabrow[e] = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+      const u32 ic = idx[e] < len[e] ? idx[e] : len[e] - 1;
+      const u32 ti = COLS ? s.tlo + (u32)(s.ik < 0 ? 0 : s.ik) : s.tlo + ic;   // target (row) particle (ik unset on blocks that just stopped)
+      const u32 sj = COLS ? s.slo + ic : s.slo + (u32)s.jk;            // source (column) particle
+#pragma unroll
+      for (int d = 0; d < 3; ++d) { xi[e][d] = A.Xs[3 * (size_t)ti + d]; xj[e][d] = A.Xs[3 * (size_t)sj + d]; }
+    }
+    entry2_eval<2>(sw, A.a, xi, xj, v);
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const BlkState& s = A.st[bb[e]];
+      const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
+      const int k = kk[e];
+      float* acc = A.acc + (size_t)bb[e] * acc_stride(A.R);
+      float bkk[9];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) bkk[r] = 0.f;
+      // residual: subtract sum_p C_p(row) Q_p(col); the fixed operand is a broadcast load
+      for (int p = 0; p < k; ++p) {
+        const float* base = chunk_ptr(A, tabrow[e], p);
+        const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
+        const float* Qp = base + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
+        float cp[9], qp[9];
+        if (ok[e]) {
+#pragma unroll
+          for (int r = 0; r < 9; ++r) {
+            cp[r] = Cp[(size_t)r * mp + (COLS ? (u32)s.ik : idx[e])];
+            qp[r] = Qp[(size_t)r * np + (COLS ? idx[e] : (u32)s.jk)];
+          }
+          submul33(v[e], cp, qp);
+        }
+      }
+      if (!ok[e]) {
+#pragma unroll
+        for (int r = 0; r < 9; ++r) v[e][r] = 0.f;
+      }
+      // store the raw residual (column: normalised later by k2_norm; row: kept raw, listing line 7)
+      float* dst = chunk_ptr(A, tabrow[e], k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np : (size_t)(k % HH_RC) * 9 * mp);
+      if (ok[e]) {
+#pragma unroll
+        for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp[e] + idx[e]] = v[e][r];
+      } else if (COLS && 4 * tile + 2 * e + half < count && s.status == 0 && idx[e] < lenp[e]) {
+#pragma unroll
+        for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp[e] + idx[e]] = 0.f;        // zero the pad columns (far kernel reads float4)
+      }
+      // arg-max scores over unused rows / columns (Eq. (9); S-18)
+      unsigned long long kd = 0ull, kf = 0ull;
+      if (ok[e]) {
+        const int* piv = a2_piv(A, bb[e]) + (COLS ? HH_MAX_RANK : 0);
+        bool used = false;
+        for (int q = 0; q < k + (COLS ? 1 : 0); ++q) used |= (piv[q] == (int)idx[e]);
+        if (!used) { kd = amax_key(fabsf(det33(v[e])), idx[e]); kf = amax_key(fro2_33(v[e]), idx[e]); }
+      }
+      kd = half_max(kd); kf = half_max(kf);
+      if (l16 == 0 && (kd | kf)) {
+        atomicMax(&A.amax[(size_t)bb[e] * 4 + (COLS ? 2 : 0)], kd);
+        atomicMax(&A.amax[(size_t)bb[e] * 4 + (COLS ? 3 : 1)], kf);
+      }
+      if (COLS) {
+        // Gram matrices of the row side (S-19): B_kk = sum_j q q^T, B_kp = sum_j q Q_p(j)^T
+        const bool any = __any_sync(0xffffffffu, ok[e]);
+        if (any) {
+#pragma unroll
+          for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+              bkk[3 * r + c] = v[e][3 * r] * v[e][3 * c] + v[e][3 * r + 1] * v[e][3 * c + 1] + v[e][3 * r + 2] * v[e][3 * c + 2];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) { float t = half_sum(bkk[r]); if (l16 == 0 && ok[e]) atomicAdd(&acc[9 + r], t); }
+          const int kmx = max(kk[0], kk[1]);                         // warp-uniform trip count for the shuffles
+          for (int p = 0; p < kmx; ++p) {
+            float bp[9];
+#pragma unroll
+            for (int r = 0; r < 9; ++r) bp[r] = 0.f;
+            if (ok[e] && p < k) {
+              const float* Qp = chunk_ptr(A, tabrow[e], p) + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
+              float qp[9];
+#pragma unroll
+              for (int r = 0; r < 9; ++r) qp[r] = Qp[(size_t)r * np + idx[e]];
+#pragma unroll
+              for (int r = 0; r < 3; ++r)
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                  bp[3 * r + c] = v[e][3 * r] * qp[3 * c] + v[e][3 * r + 1] * qp[3 * c + 1] + v[e][3 * r + 2] * qp[3 * c + 2];
+            }
+#pragma unroll
+            for (int r = 0; r < 9; ++r) {
+              float t = half_sum(bp[r]);
+              if (l16 == 0 && ok[e] && p < k) atomicAdd(&acc[18 + 9 * (A.R + 1) + 9 * p + r], t);
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
+__device__ __forceinline__ void a2_decode(unsigned long long key, float& score, int& idx) {
+  score = key ? __uint_as_float((u32)(key >> 32)) : -1.f;
+  idx = key ? (int)(0xffffffffu - (u32)key) : -1;
+}
+// S-18: |det| rule falls back to Frobenius when every remaining |det| is 0; rule 1 = Frobenius
+__device__ __forceinline__ void a2_choose(int rule, unsigned long long kd, unsigned long long kf, int& idx, float& best) {
+  float bd, bf; int bdi, bfi;
+  a2_decode(kd, bd, bdi); a2_decode(kf, bf, bfi);
+  if (rule == 0 && (bd > 0.f || bf <= 0.f)) { idx = bdi; best = bd; } else { idx = bfi; best = bf; }
+}
+
+// ---- lines 5-6: pivot row, P^-1 and cond_F(P) in fp64 ----
+__global__ void __launch_bounds__(256) k2_piv(A2Args A) {
+  const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= A.nb) return;
+  BlkState s = A.st[b];
+  if (s.status != 0) return;
+  int ik; float best;
+  a2_choose(A.rule, A.amax[(size_t)b * 4], A.amax[(size_t)b * 4 + 1], ik, best);
+  if (ik < 0 || !(best > 0.f)) { a2_finish(A, b, s, 1, 0); A.st[b] = s; return; }   // S-21: zero residual column -> block reproduced
+  const u32 mp = a2_pad8(s.m);
+  const u32* tabrow = A.tab + (size_t)b * HH_TAB_STRIDE;
+  const float* Ck = chunk_ptr(A, tabrow, s.k) + (size_t)(s.k % HH_RC) * 9 * mp;
+  double P[9], Pi[9];
+#pragma unroll
+  for (int r = 0; r < 9; ++r) P[r] = (double)Ck[(size_t)r * mp + ik];
+  a2_piv(A, b)[s.k] = ik;
+  const double dP = P[0] * (P[4] * P[8] - P[5] * P[7]) - P[1] * (P[3] * P[8] - P[5] * P[6]) + P[2] * (P[3] * P[7] - P[4] * P[6]);
+  bool sing = fabs(dP) < 1e-30;
+  if (!sing) {
+    const double iv = 1.0 / dP;
+    Pi[0] = (P[4] * P[8] - P[5] * P[7]) * iv; Pi[1] = (P[2] * P[7] - P[1] * P[8]) * iv; Pi[2] = (P[1] * P[5] - P[2] * P[4]) * iv;
+    Pi[3] = (P[5] * P[6] - P[3] * P[8]) * iv; Pi[4] = (P[0] * P[8] - P[2] * P[6]) * iv; Pi[5] = (P[2] * P[3] - P[0] * P[5]) * iv;
+    Pi[6] = (P[3] * P[7] - P[4] * P[6]) * iv; Pi[7] = (P[1] * P[6] - P[0] * P[7]) * iv; Pi[8] = (P[0] * P[4] - P[1] * P[3]) * iv;
+    double np2 = 0.0, ni2 = 0.0;
+#pragma unroll
+    for (int r = 0; r < 9; ++r) { np2 += P[r] * P[r]; ni2 += Pi[r] * Pi[r]; }
+    sing = sqrt(np2 * ni2) > A.kappa_max;                          // S-18b
+  }
+  if (sing) { a2_finish(A, b, s, 2, 2); A.st[b] = s; return; }     // S-18 / S-18b: breakdown -> the block is applied densely
+#pragma unroll
+  for (int r = 0; r < 9; ++r) A.pinv[(size_t)b * 9 + r] = Pi[r];
+  s.ik = ik;
+  A.st[b] = s;
+}
+
+// ---- line 6: c_k(i) = c'(i) P^-1; Gram matrices A_kk, A_pk (S-19).  Half a warp per granule of rows. ----
+__global__ void __launch_bounds__(256) k2_norm(A2Args A, u32 count) {
+  const u32 lane = threadIdx.x & 31, l16 = lane & 15;
+  const u32 gi = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
+  const bool gv = gi < count;
+  const uint2 g = A.gm[gv ? gi : count - 1];
+  const BlkState& s = A.st[g.x];
+  const u32 i = g.y + l16, mp = a2_pad8(s.m);
+  const bool ok = gv && s.status == 0 && i < s.m;
+  const int k = s.k;
+  const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+  float* acc = A.acc + (size_t)g.x * acc_stride(A.R);
+  float c[9], akk[9];
+#pragma unroll
+  for (int r = 0; r < 9; ++r) { c[r] = 0.f; akk[r] = 0.f; }
+  if (ok) {
+    float* Ck = chunk_ptr(A, tabrow, k) + (size_t)(k % HH_RC) * 9 * mp;
+    double Pi[9];
+    float cr[9];
+#pragma unroll
+    for (int r = 0; r < 9; ++r) { Pi[r] = A.pinv[(size_t)g.x * 9 + r]; cr[r] = Ck[(size_t)r * mp + i]; }
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int q = 0; q < 3; ++q)
+        c[3 * r + q] = (float)((double)cr[3 * r] * Pi[q] + (double)cr[3 * r + 1] * Pi[3 + q] + (double)cr[3 * r + 2] * Pi[6 + q]);
+#pragma unroll
+    for (int r = 0; r < 9; ++r) Ck[(size_t)r * mp + i] = c[r];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int q = 0; q < 3; ++q) akk[3 * r + q] = c[r] * c[q] + c[3 + r] * c[3 + q] + c[6 + r] * c[6 + q];
+  }
+#pragma unroll
+  for (int r = 0; r < 9; ++r) { float t = half_sum(akk[r]); if (l16 == 0 && ok) atomicAdd(&acc[r], t); }
+  const int ko = ok ? k : 0;
+  const int kmx = max(ko, __shfl_xor_sync(0xffffffffu, ok ? k : 0, 16));
+  int kw = kmx;                                                   // warp-uniform trip count (both halves, all lanes)
+#pragma unroll
+  for (int o = 8; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
+  for (int p = 0; p < kw; ++p) {
+    float ap[9];
+#pragma unroll
+    for (int r = 0; r < 9; ++r) ap[r] = 0.f;
+    if (ok && p < k) {
+      const float* Cp = chunk_ptr(A, tabrow, p) + (size_t)(p % HH_RC) * 9 * mp;
+      float cp[9];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + i];
+#pragma unroll
+      for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int q = 0; q < 3; ++q) ap[3 * r + q] = cp[r] * c[q] + cp[3 + r] * c[3 + q] + cp[6 + r] * c[6 + q];
+    }
+#pragma unroll
+    for (int r = 0; r < 9; ++r) { float t = half_sum(ap[r]); if (l16 == 0 && ok && p < k) atomicAdd(&acc[18 + 9 * p + r], t); }
+  }
+}
+
+// ---- lines 9-12: norm recursion (S-19), stop test Eq. (10) (S-20), next column (line 8), arena space ----
+__global__ void __launch_bounds__(256) k2_fin(A2Args A) {
+  const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= A.nb) return;
+  BlkState s = A.st[b];
+  if (s.status != 0) return;
+  const float* acc = A.acc + (size_t)b * acc_stride(A.R);
+  const int k = s.k;
+  float nu2 = 0.f, cross = 0.f;
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int q = 0; q < 3; ++q) nu2 = fmaf(acc[3 * r + q], acc[9 + 3 * q + r], nu2);               // tr(A_kk B_kk)
+  for (int p = 0; p < k; ++p) {
+    const float* Ap = acc + 18 + 9 * p;
+    const float* Bp = acc + 18 + 9 * (A.R + 1) + 9 * p;
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int q = 0; q < 3; ++q) cross = fmaf(Ap[3 * r + q], Bp[3 * q + r], cross);               // tr(A_pk B_kp)
+  }
+  s.lam2 += nu2 + 2.f * cross;
+  s.k = k + 1;
+  const float nu = sqrtf(fmaxf(nu2, 0.f)), lam = sqrtf(fmaxf(s.lam2, 0.f));
+  if (nu <= A.tol * lam) { a2_finish(A, b, s, 1, 0); A.st[b] = s; return; }                        // Eq. (10)
+  int jn; float best;
+  a2_choose(A.rule, A.amax[(size_t)b * 4 + 2], A.amax[(size_t)b * 4 + 3], jn, best);
+  if (jn < 0) { a2_finish(A, b, s, 1, 0); A.st[b] = s; return; }
+  if (s.k >= s.kmax) {                                                                             // S-21: N_ite_max reached (flag 1) or min(c,q): exact
+    a2_finish(A, b, s, 1, s.kmax < min((int)s.m, (int)s.n) ? 1 : 0);
+    A.st[b] = s;
+    return;
+  }
+  s.jk = jn;
+  a2_piv(A, b)[HH_MAX_RANK + s.k] = jn;
+  if ((s.k % HH_RC) == 0 && !a2_alloc(A, b, s, s.k)) s.status = -1;     // arena full: this block is redone in the next batch
+  else a2_zero_acc(A, b, s.k);
+  A.st[b] = s;
+}
+
+// largest `end` such that blocks [first, end) fit the scratch region at the predicted number of chunks per block,
+// including the lock-step state (table row, block state, accumulators, granule lists)
+__global__ void k2_batch_range(const u64* __restrict__ unit_prefix, u32 first, u32 nG, u64 total_units, u32 chunks_pred,
+                               u32 per_block_units, DevScalars* sc) {
+  u32 lo = first, hi = nG;
+  const u64 s0 = unit_prefix[first];
+  while (lo < hi) {
+    u32 mid = lo + (hi - lo + 1) / 2;
+    const u64 rows = unit_prefix[mid] - s0;
+    u64 need = rows * 9ull / 8ull * chunks_pred + (u64)(mid - first) * (7ull + per_block_units) + rows / 8ull + 64ull;
+    if (need <= total_units) lo = mid; else hi = mid - 1;
+  }
+  sc->batch_end = lo;
+  sc->batch_units = unit_prefix[lo] - s0;
+  sc->batch_units1 = unit_prefix[first + 1 <= nG ? first + 1 : first] - s0;
+  sc->arena_cursor = 0;
+  sc->fail_min = 0xffffffffu;
+  sc->sum_rank = sc->aca_entries = sc->factor_bytes = 0;
+  sc->not_conv = sc->singular = sc->max_rank_seen = 0;
+  sc->n_dense = 0;
+  sc->fallback_entries = 0;
+}
+
+static size_t a2_align(size_t v) { return (v + 255) / 256 * 256; }
+
+int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
+  cudaStream_t s = ctx->stream;
+  const u32 nG = (u32)ctx->nG;
+  const int R = ctx->p.aca_max_rank;
+  u32 chunks_pred = (u32)((ctx->l_pred + HH_RC - 1) / HH_RC);
+  if (chunks_pred < 1) chunks_pred = 1;
+  if (chunks_pred > HH_MAX_CHUNKS) chunks_pred = HH_MAX_CHUNKS;
+  // per block: table row 128 B, state 64 B, arg-max keys 32 B, P^-1 72 B, accumulators, 2 counters, 2 granules of slack
+  const size_t acc_floats = 18 + 18 * (size_t)(R + 1);
+  const size_t per_block_bytes = 128 + 64 + 32 + 72 + 4 * acc_floats + 8 + 32 + 16;
+  const u32 per_block_units = (u32)((per_block_bytes + 127) / 128);
+  const u64 total_units = ctx->scratch_bytes / 128;
+  u32 end_cap = nG;
+  for (int attempt = 0; attempt < 24; ++attempt) {
+    k2_batch_range<<<HH_N + 1, 1, 0, s>>>(ctx->unit_prefix, (u32)first, end_cap, total_units > 64 ? total_units - 64 : 0, chunks_pred,
+                                          per_block_units, ctx->d_sc);
+    HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
+    HH_CUDA(cudaStreamSynchronize(s));
+    u32 end = ctx->h_sc->batch_end;
+    u64 rows = ctx->h_sc->batch_units;
+    if (end <= first) { end = (u32)first + 1; rows = ctx->h_sc->batch_units1; }   // try a single block; it fails below if it cannot fit
+    const u32 nb = end - (u32)first;
+    const size_t ngran = (size_t)(rows / GR) + nb + 8;                           // bound on the granules of either list
+    // carve the scratch region: lock-step state first, the arena after it
+    char* p = ctx->scratch;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { char* r = p + off; off = a2_align(off + bytes); return r; };
+    ctx->tab = (u32*)take((size_t)nb * HH_TAB_STRIDE * sizeof(u32));
+    A2Args A;
+    A.st = (BlkState*)take((size_t)nb * sizeof(BlkState));
+    A.amax = (unsigned long long*)take((size_t)nb * 4 * sizeof(unsigned long long));
+    A.pinv = (double*)take((size_t)nb * 9 * sizeof(double));
+    A.acc = (float*)take((size_t)nb * acc_floats * sizeof(float));
+    A.cm = (u32*)take((size_t)(nb + 1) * sizeof(u32));
+    A.cn = (u32*)take((size_t)(nb + 1) * sizeof(u32));
+    A.gm = (uint2*)take(ngran * sizeof(uint2));
+    A.gn = (uint2*)take(ngran * sizeof(uint2));
+    if (off + 4096 > ctx->scratch_bytes) return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "factor arena too small");
+    ctx->arena = (float*)(ctx->scratch + off);
+    ctx->arena_units = (ctx->scratch_bytes - off) / 128;
+    A.w2 = ctx->w2; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.rule = ctx->p.pivot_rule;
+    A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : 300.0;
+    A.PG = ctx->PG; A.nlo = ctx->nlo; A.nhi = ctx->nhi; A.Xs = ctx->Xs;
+    A.arena = ctx->arena; A.arena_units = ctx->arena_units; A.tab = ctx->tab; A.sc = ctx->d_sc;
+    A.ranks = ctx->ranks; A.flags = ctx->flags; A.first = (u32)first; A.nb = nb; A.R = R;
+    const unsigned gb = cdiv(nb, 256);
+    k2_init<<<HH_N + gb, 256, 0, s>>>(A);
+    HH_LAUNCH_CHECK();
+    for (int it = 0; it <= R; ++it) {
+      HH_CUDA(cudaMemsetAsync(&ctx->d_sc->n_split, 0, sizeof(u32), s));
+      k2_gran_count<<<HH_N + gb, 256, 0, s>>>(A);
+      HH_TRY(hh_scan_u32(ctx, A.cm, A.cm, nb, &ctx->d_sc->lvl.g));
+      HH_TRY(hh_scan_u32(ctx, A.cn, A.cn, nb, &ctx->d_sc->lvl.h));
+      HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->n_split, &ctx->d_sc->n_split, sizeof(u32), cudaMemcpyDeviceToHost, s));
+      HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->lvl, &ctx->d_sc->lvl, sizeof(Cnt3), cudaMemcpyDeviceToHost, s));
+      HH_CUDA(cudaStreamSynchronize(s));
+      const u32 nact = ctx->h_sc->n_split, gmc = ctx->h_sc->lvl.g, gnc = ctx->h_sc->lvl.h;
+      if (nact == 0) break;
+      if (gmc > ngran || gnc > ngran) return hh_fail(ctx, HH_ERR_CUDA, "lock-step ACA: granule list overflow (internal)");
+      k2_gran_fill<<<HH_N + cdiv((int64_t)nb * 32, 256), 256, 0, s>>>(A);
+      const unsigned cap = 148 * 2 * 4;
+      unsigned g1 = cdiv(cdiv(gmc, 4), A2_T / 32), g2 = cdiv(cdiv(gnc, 4), A2_T / 32);
+      k2_eval<false><<<HH_N + (g1 < cap ? g1 : cap), A2_T, 0, s>>>(A, gmc);
+      k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
+      k2_norm<<<HH_N + cdiv((int64_t)gmc * GR, 256), 256, 0, s>>>(A, gmc);
+      k2_eval<true><<<HH_N + (g2 < cap ? g2 : cap), A2_T, 0, s>>>(A, gnc);
+      k2_fin<<<HH_N + gb, 256, 0, s>>>(A);
+      HH_LAUNCH_CHECK();
+    }
+    // blocks drop out in rank order, not in list order: when the arena overflows the first failed block can sit early
+    // in the batch.  Then most of the batch would be discarded -- shrink the batch and run it again instead.
+    HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->fail_min, &ctx->d_sc->fail_min, sizeof(u32), cudaMemcpyDeviceToHost, s));
+    HH_CUDA(cudaStreamSynchronize(s));
+    const u32 fm = ctx->h_sc->fail_min;
+    if (fm < end && nb > 1 && (fm - (u32)first) < nb - nb / 4) {
+      end_cap = (u32)first + (nb / 2 > 1 ? nb / 2 : 1);
+      ctx->l_pred = ctx->l_pred * 1.25 > HH_MAX_RANK ? HH_MAX_RANK : ctx->l_pred * 1.25;
+      continue;
+    }
+    return hh_aca_batch_finish(ctx, first, end, next);
+  }
+  return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "lock-step ACA: could not fit a batch into the factor arena");
+}

@@ -42,7 +42,7 @@ static int carve(hh_ctx* ctx, int64_t N) {
   ctx->near_begin = c.take<u32>(nodes); ctx->near_end = c.take<u32>(nodes);
   ctx->PG = c.take<uint2>(ctx->cap_pairs); ctx->PH = c.take<uint2>(ctx->cap_pairs);
   ctx->ranks = c.take<int>(ctx->cap_pairs); ctx->flags = c.take<int>(ctx->cap_pairs);
-  ctx->dense_list = c.take<u32>(ctx->cap_pairs);
+  ctx->dense_list = c.take<u32>(ctx->cap_pairs); ctx->dense_cnt = c.take<u32>(ctx->cap_pairs + 1);
   ctx->unit_prefix = c.take<u64>(ctx->cap_pairs + 1);
   ctx->n_cells_cap = 4 * N + 4096;
   ctx->cell_of = c.take<u32>(N); ctx->cell_order = c.take<u32>(N); ctx->cell_start = c.take<u32>(ctx->n_cells_cap + 1);
@@ -197,6 +197,14 @@ extern "C" int hh_set_pair_capacity(hh_ctx* ctx, int64_t pairs_per_particle) {
   return HH_OK;
 }
 
+// 0 = lock-step over the batch (default), 1 = one CTA per admissible block (the first form; kept for comparison)
+extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
+  if (!ctx || (impl != 0 && impl != 1)) return HH_ERR_INVALID_ARG;
+  ctx->aca_impl = impl;
+  ctx->res_first = ctx->res_next = 0;
+  return HH_OK;
+}
+
 extern "C" int hh_enable_timing(hh_ctx* ctx, int on) {
   if (!ctx) return HH_ERR_INVALID_ARG;
   ctx->timing = on;
@@ -242,7 +250,7 @@ extern "C" int hh_aca(hh_ctx* ctx, int64_t first_block, int64_t* next_block) {
   if (first_block < 0 || first_block > ctx->nG) return hh_fail(ctx, HH_ERR_INVALID_ARG, "hh_aca: first_block out of range");
   if (first_block == ctx->nG) { *next_block = ctx->nG; ctx->res_first = ctx->res_next = ctx->nG; return HH_OK; }
   T0(2);
-  HH_TRY(hh_aca_batch(ctx, first_block, next_block));
+  HH_TRY(ctx->aca_impl == 1 ? hh_aca_batch(ctx, first_block, next_block) : hh_aca2_batch(ctx, first_block, next_block));
   T0(3);
   if (ctx->timing) ctx->st.ms_aca += ev_ms(ctx, 2, 3);
   return HH_OK;

@@ -48,6 +48,7 @@ struct DevScalars {
   u64 near_entries, far_rows_cols;
   u32 max_rank_seen, n_dense;
   u64 fallback_entries;
+  u64 batch_units, batch_units1;  /* lock-step ACA: padded rows + columns of the batch [first, batch_end) resp. of block `first` alone */
 };
 
 struct hh_ctx {
@@ -57,6 +58,7 @@ struct hh_ctx {
   char err[512];
   int have_mlp3;
   int timing;
+  int aca_impl;                         /* 0 = lock-step (hh_aca2.cu), 1 = one CTA per block (hh_aca.cu) */
   int64_t pairs_per_particle;
   /* state */
   int64_t N, Ncap;
@@ -86,7 +88,7 @@ struct hh_ctx {
   uint2 *PG, *PH;                       /* (tau, sigma) node ids; PG sorted by size desc, PH by tau */
   u32 *near_begin, *near_end;           /* per node: range in PH                              */
   int* ranks; int* flags;               /* per admissible block                               */
-  u32* dense_list; u32 n_dense;         /* resident blocks on which Alg. 2 broke down (S-18b): applied densely */
+  u32* dense_list; u32* dense_cnt; u32 n_dense;         /* resident blocks on which Alg. 2 broke down (S-18b): applied densely */
   u64* unit_prefix;                     /* prefix of (m_pad + n_pad) over sorted PG, nG+1     */
   char* scratch; size_t scratch_bytes;  /* frontier ping-pong during build; == arena region    */
   float* arena; u64 arena_units;        /* after the resident table                            */
@@ -129,7 +131,9 @@ int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N);
 int hh_blocks_build(hh_ctx* ctx);
 int hh_near_apply(hh_ctx* ctx);                                       /* Us += near-field           */
 int hh_dense_apply(hh_ctx* ctx);                                      /* Us += resident blocks on which ACA broke down, densely */
-int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next);
+int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next);      /* one CTA per block (hh_aca.cu)        */
+int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next);     /* lock-step over the batch (hh_aca2.cu) */
+int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next);   /* stats, dense list, rank prediction */
 int hh_far_apply(hh_ctx* ctx);                                        /* Us += resident far-field   */
 int hh_three_apply(hh_ctx* ctx);                                     /* Us += three-body term (tree order) */
 int hh_entries_eval(hh_ctx* ctx, const float* Xi, const float* Xj, int64_t n, float* M);

@@ -92,49 +92,62 @@ int hh_near_apply(hh_ctx* ctx) {
 }
 
 // S-18b: admissible blocks on which Alg. 2 broke down (numerically singular pivot) are evaluated densely, exactly
-// like the inadmissible ones (L252).  One CTA per such block; rows in tiles of HH_MAX_LEAF, sources in tiles of NR_TILE.
-__global__ void __launch_bounds__(NR_T) k_dense(const float* __restrict__ gw, float a, const u32* __restrict__ list,
-                                                 const uint2* __restrict__ PG, const u32* __restrict__ nlo, const u32* __restrict__ nhi,
-                                                 const float* __restrict__ Xs, const float* __restrict__ Fs, float* __restrict__ Us) {
+// like the inadmissible ones (L252).  Each such block is cut into tiles of HH_MAX_LEAF rows x NR_TILE columns; the tiles
+// of all blocks form one flat list (prefix over the blocks, binary search per CTA), so a 4096 x 4096 block spreads
+// over the whole GPU instead of one SM.
+__global__ void __launch_bounds__(256) k_dense_count(const u32* __restrict__ list, u32 n, const uint2* __restrict__ PG,
+                                                      const u32* __restrict__ nlo, const u32* __restrict__ nhi, u32* __restrict__ cnt) {
+  u32 t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const uint2 blk = PG[list[t]];
+  const u32 m = nhi[blk.x] - nlo[blk.x], q = nhi[blk.y] - nlo[blk.y];
+  cnt[t] = ((m + HH_MAX_LEAF - 1) / HH_MAX_LEAF) * ((q + NR_TILE - 1) / NR_TILE);
+}
+
+__global__ void __launch_bounds__(NR_T, 2) k_dense(const float* __restrict__ gw, float a, const u32* __restrict__ list, u32 n_list,
+                                                    const u32* __restrict__ tile_prefix, const u32* __restrict__ total_tiles,
+                                                    const uint2* __restrict__ PG, const u32* __restrict__ nlo, const u32* __restrict__ nhi,
+                                                    const float* __restrict__ Xs, const float* __restrict__ Fs, float* __restrict__ Us) {
   __shared__ __align__(16) float sw[HH_MLP2_FLOATS];
   __shared__ float tX[HH_MAX_LEAF * 3], sU[HH_MAX_LEAF * 3];
   __shared__ float sXj[NR_TILE * 3], sFj[NR_TILE * 3];
   const u32 tid = threadIdx.x;
-  const uint2 blk = PG[list[blockIdx.x]];
-  const u32 tlo = nlo[blk.x], m = nhi[blk.x] - tlo;
-  const u32 slo = nlo[blk.y], n = nhi[blk.y] - slo;
   load_weights(sw, gw, HH_MLP2_FLOATS);
-  for (u32 r0 = 0; r0 < m; r0 += HH_MAX_LEAF) {
-    const u32 mt = min((u32)HH_MAX_LEAF, m - r0);
+  const u32 total = *total_tiles;
+  for (u32 tile = blockIdx.x; tile < total; tile += gridDim.x) {
+    u32 lo = 0, hi = n_list - 1;                                   // last block whose first tile is <= tile
+    while (lo < hi) { u32 mid = (lo + hi + 1) / 2; if (tile_prefix[mid] <= tile) lo = mid; else hi = mid - 1; }
+    const uint2 blk = PG[list[lo]];
+    const u32 tlo = nlo[blk.x], m = nhi[blk.x] - tlo;
+    const u32 slo = nlo[blk.y], n = nhi[blk.y] - slo;
+    const u32 ct = (n + NR_TILE - 1) / NR_TILE, local = tile - tile_prefix[lo];
+    const u32 r0 = (local / ct) * HH_MAX_LEAF, j0 = (local % ct) * NR_TILE;
+    const u32 mt = min((u32)HH_MAX_LEAF, m - r0), nt = min((u32)NR_TILE, n - j0);
     __syncthreads();
     for (u32 t = tid; t < 3 * mt; t += NR_T) { tX[t] = Xs[3 * (size_t)(tlo + r0) + t]; sU[t] = 0.f; }
-    for (u32 j0 = 0; j0 < n; j0 += NR_TILE) {
-      const u32 nt = min((u32)NR_TILE, n - j0);
-      __syncthreads();
-      for (u32 t = tid; t < 3 * nt; t += NR_T) { sXj[t] = Xs[3 * (size_t)(slo + j0) + t]; sFj[t] = Fs[3 * (size_t)(slo + j0) + t]; }
-      __syncthreads();
-      const u32 pairs = mt * nt;
-      for (u32 p0 = tid; p0 < pairs; p0 += 2 * NR_T) {
-        u32 pp[2] = {p0, p0 + NR_T};
-        bool ok[2] = {true, pp[1] < pairs};
-        if (!ok[1]) pp[1] = p0;
-        u32 ii[2], jj[2];
-        float xi[2][3], xj[2][3], M[2][9];
+    for (u32 t = tid; t < 3 * nt; t += NR_T) { sXj[t] = Xs[3 * (size_t)(slo + j0) + t]; sFj[t] = Fs[3 * (size_t)(slo + j0) + t]; }
+    __syncthreads();
+    const u32 pairs = mt * nt;
+    for (u32 p0 = tid; p0 < pairs; p0 += 2 * NR_T) {
+      u32 pp[2] = {p0, p0 + NR_T};
+      bool ok[2] = {true, pp[1] < pairs};
+      if (!ok[1]) pp[1] = p0;
+      u32 ii[2], jj[2];
+      float xi[2][3], xj[2][3], M[2][9];
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          jj[e] = pp[e] / mt; ii[e] = pp[e] - jj[e] * mt;
+      for (int e = 0; e < 2; ++e) {
+        jj[e] = pp[e] / mt; ii[e] = pp[e] - jj[e] * mt;
 #pragma unroll
-          for (int c = 0; c < 3; ++c) { xi[e][c] = tX[3 * ii[e] + c]; xj[e][c] = sXj[3 * jj[e] + c]; }
-        }
-        entry2_eval<2>(sw, a, xi, xj, M);
+        for (int c = 0; c < 3; ++c) { xi[e][c] = tX[3 * ii[e] + c]; xj[e][c] = sXj[3 * jj[e] + c]; }
+      }
+      entry2_eval<2>(sw, a, xi, xj, M);
 #pragma unroll
-        for (int e = 0; e < 2; ++e) {
-          if (ok[e] && tlo + r0 + ii[e] != slo + j0 + jj[e]) {
-            const float f0 = sFj[3 * jj[e]], f1 = sFj[3 * jj[e] + 1], f2 = sFj[3 * jj[e] + 2];
+      for (int e = 0; e < 2; ++e) {
+        if (ok[e] && tlo + r0 + ii[e] != slo + j0 + jj[e]) {
+          const float f0 = sFj[3 * jj[e]], f1 = sFj[3 * jj[e] + 1], f2 = sFj[3 * jj[e] + 2];
 #pragma unroll
-            for (int al = 0; al < 3; ++al)
-              atomicAdd(&sU[3 * ii[e] + al], fmaf(M[e][3 * al], f0, fmaf(M[e][3 * al + 1], f1, M[e][3 * al + 2] * f2)));
-          }
+          for (int al = 0; al < 3; ++al)
+            atomicAdd(&sU[3 * ii[e] + al], fmaf(M[e][3 * al], f0, fmaf(M[e][3 * al + 1], f1, M[e][3 * al + 2] * f2)));
         }
       }
     }
@@ -145,8 +158,12 @@ __global__ void __launch_bounds__(NR_T) k_dense(const float* __restrict__ gw, fl
 
 int hh_dense_apply(hh_ctx* ctx) {
   if (ctx->res_next <= ctx->res_first || ctx->n_dense == 0) return HH_OK;
-  k_dense<<<HH_N + ctx->n_dense, NR_T, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, ctx->dense_list, ctx->PG, ctx->nlo, ctx->nhi,
-                                                        ctx->Xs, ctx->Fs, ctx->Us);
+  const u32 n = ctx->n_dense;
+  u32* cnt = ctx->dense_cnt;
+  k_dense_count<<<HH_N + cdiv(n, 256), 256, 0, ctx->stream>>>(ctx->dense_list, n, ctx->PG, ctx->nlo, ctx->nhi, cnt);
+  HH_TRY(hh_scan_u32(ctx, cnt, cnt, n, &ctx->d_sc->n_split));
+  k_dense<<<HH_N + 148 * 2, NR_T, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, ctx->dense_list, n, cnt, &ctx->d_sc->n_split, ctx->PG,
+                                                    ctx->nlo, ctx->nhi, ctx->Xs, ctx->Fs, ctx->Us);
   HH_LAUNCH_CHECK();
   return HH_OK;
 }

@@ -11,8 +11,9 @@
 //   k_piv   line 5-6  pivot row i_k, P = c'(i_k), P^-1 and cond_F(P) in fp64; zero column -> done (S-21); singular or
 //                     cond_F > kappa_max -> breakdown, block goes dense (S-18, S-18b)
 //   k_norm  line 6    c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk, A_pk = sum_i C_p(i)^T c_k(i)   (S-19)
-//   k_row   line 7-8  q_k(j) = G(i_k,j) - sum_p C_p(i_k) Q_p(j), stored raw; arg-max for j_{k+1}; B_kk, B_kp = sum_j q_k(j) Q_p(j)^T
-//   k_fin   line 9-12 nu^2 = tr(A_kk B_kk), lambda^2 += nu^2 + 2 sum_p tr(A_pk B_kp); stop test Eq. (10) (S-20);
+//   k_row   line 7-8  q_k(j) = G(i_k,j) - sum_p C_p(i_k) Q_p(j), stored raw; arg-max for j_{k+1};
+//                     nu^2 = sum_j tr(A_kk q q^T), cross = sum_j tr([sum_p Q_p(j)^T A_pk] q(j))  (= sum_p tr(A_pk B_kp), S-19)
+//   k_fin   line 9-12 lambda^2 += nu^2 + 2 cross; stop test Eq. (10) (S-20);
 //                     next column; arena space for the next HH_RC ranks
 // Storage, arena chunks, table rows and the pivot record are those of hh_aca.cu (the far-field kernel reads both).
 #include "hh_mlp.cuh"
@@ -43,8 +44,8 @@ struct A2Args {
 };
 
 __device__ __forceinline__ u32 a2_pad8(u32 v) { return (v + 7u) & ~7u; }
-__device__ __forceinline__ int acc_stride(int R) { return 18 + 18 * (R + 1); }
-/* accumulators of a block: [0,9) A_kk, [9,18) B_kk, 18 + 9p: A_pk, 18 + 9(R+1) + 9p: B_kp                 */
+__device__ __forceinline__ int acc_stride(int R) { return 18 + 9 * (R + 1); }
+/* accumulators of a block: [0,9) A_kk, [9] nu^2, [10] cross term, 18 + 9p: A_pk                          */
 __device__ __forceinline__ float* chunk_ptr(const A2Args& A, const u32* tabrow, int p) {
   return A.arena + (size_t)tabrow[p / HH_RC] * HH_UNIT_FLOATS;
 }
@@ -55,6 +56,25 @@ __device__ __forceinline__ float half_sum(float v) {                            
 #pragma unroll
   for (int o = 8; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
+}
+// Sum 9 values over the 16 lanes of a half-warp with 15 shuffles (halving butterfly): on return lane l (l < 9) of the
+// half-warp holds the total of v[l] in v[0].
+__device__ __forceinline__ float half_sum9(const float (&in)[9], u32 l16) {
+  float v[16];
+#pragma unroll
+  for (int r = 0; r < 9; ++r) v[r] = in[r];
+#pragma unroll
+  for (int r = 9; r < 16; ++r) v[r] = 0.f;
+#pragma unroll
+  for (int w = 8; w; w >>= 1) {
+    const bool up = (l16 & w) != 0;
+#pragma unroll
+    for (int r = 0; r < w; ++r) {
+      const float send = up ? v[r] : v[r + w], keep = up ? v[r + w] : v[r];
+      v[r] = keep + __shfl_xor_sync(0xffffffffu, send, w);
+    }
+  }
+  return v[0];
 }
 __device__ __forceinline__ unsigned long long half_max(unsigned long long v) {
 #pragma unroll
@@ -80,7 +100,7 @@ __device__ __forceinline__ int* a2_piv(const A2Args& A, u32 b) {
 __device__ __forceinline__ void a2_zero_acc(const A2Args& A, u32 b, int k) {      // slots used by step k
   float* acc = A.acc + (size_t)b * acc_stride(A.R);
   for (int t = 0; t < 18; ++t) acc[t] = 0.f;
-  for (int t = 0; t < 9 * k; ++t) { acc[18 + t] = 0.f; acc[18 + 9 * (A.R + 1) + t] = 0.f; }
+  for (int t = 0; t < 9 * k; ++t) acc[18 + t] = 0.f;
   for (int t = 0; t < 4; ++t) A.amax[(size_t)b * 4 + t] = 0ull;
 }
 __device__ __forceinline__ void a2_finish(const A2Args& A, u32 b, BlkState& s, int status, int flag) {
@@ -172,9 +192,6 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
       const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
       const int k = kk[e];
       float* acc = A.acc + (size_t)bb[e] * acc_stride(A.R);
-      float bkk[9];
-#pragma unroll
-      for (int r = 0; r < 9; ++r) bkk[r] = 0.f;
       // residual: subtract sum_p C_p(row) Q_p(col); the fixed operand is a broadcast load
       for (int p = 0; p < k; ++p) {
         const float* base = chunk_ptr(A, tabrow[e], p);
@@ -217,39 +234,32 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
         atomicMax(&A.amax[(size_t)bb[e] * 4 + (COLS ? 3 : 1)], kf);
       }
       if (COLS) {
-        // Gram matrices of the row side (S-19): B_kk = sum_j q q^T, B_kp = sum_j q Q_p(j)^T
-        const bool any = __any_sync(0xffffffffu, ok[e]);
-        if (any) {
+        // norm recursion (S-19) with the column-side Gram matrices of k2_norm, which ran before this kernel:
+        //   nu^2 = sum_j tr(A_kk q q^T),  cross = sum_p tr(A_pk B_kp) = sum_j tr( [sum_p Q_p(j)^T A_pk] q(j) )
+        float nu2 = 0.f, cross = 0.f;
+        if (ok[e]) {
+          float W[9], Z[9];
+          mul33(acc, v[e], W);
+#pragma unroll
+          for (int r = 0; r < 9; ++r) { nu2 = fmaf(W[r], v[e][r], nu2); Z[r] = 0.f; }
+          for (int p = 0; p < k; ++p) {
+            const float* Qp = chunk_ptr(A, tabrow[e], p) + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
+            const float* Ap = acc + 18 + 9 * p;
+            float qp[9];
+#pragma unroll
+            for (int r = 0; r < 9; ++r) qp[r] = Qp[(size_t)r * np + idx[e]];
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int c = 0; c < 3; ++c) Z[3 * r + c] += qp[r] * Ap[c] + qp[3 + r] * Ap[3 + c] + qp[6 + r] * Ap[6 + c];
+          }
 #pragma unroll
           for (int r = 0; r < 3; ++r)
 #pragma unroll
-            for (int c = 0; c < 3; ++c)
-              bkk[3 * r + c] = v[e][3 * r] * v[e][3 * c] + v[e][3 * r + 1] * v[e][3 * c + 1] + v[e][3 * r + 2] * v[e][3 * c + 2];
-#pragma unroll
-          for (int r = 0; r < 9; ++r) { float t = half_sum(bkk[r]); if (l16 == 0 && ok[e]) atomicAdd(&acc[9 + r], t); }
-          const int kmx = max(kk[0], kk[1]);                         // warp-uniform trip count for the shuffles
-          for (int p = 0; p < kmx; ++p) {
-            float bp[9];
-#pragma unroll
-            for (int r = 0; r < 9; ++r) bp[r] = 0.f;
-            if (ok[e] && p < k) {
-              const float* Qp = chunk_ptr(A, tabrow[e], p) + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
-              float qp[9];
-#pragma unroll
-              for (int r = 0; r < 9; ++r) qp[r] = Qp[(size_t)r * np + idx[e]];
-#pragma unroll
-              for (int r = 0; r < 3; ++r)
-#pragma unroll
-                for (int c = 0; c < 3; ++c)
-                  bp[3 * r + c] = v[e][3 * r] * qp[3 * c] + v[e][3 * r + 1] * qp[3 * c + 1] + v[e][3 * r + 2] * qp[3 * c + 2];
-            }
-#pragma unroll
-            for (int r = 0; r < 9; ++r) {
-              float t = half_sum(bp[r]);
-              if (l16 == 0 && ok[e] && p < k) atomicAdd(&acc[18 + 9 * (A.R + 1) + 9 * p + r], t);
-            }
-          }
+            for (int c = 0; c < 3; ++c) cross = fmaf(Z[3 * r + c], v[e][3 * c + r], cross);
         }
+        nu2 = half_sum(nu2); cross = half_sum(cross);
+        if (l16 == 0 && ok[e]) { atomicAdd(&acc[9], nu2); atomicAdd(&acc[10], cross); }
       }
     }
   }
@@ -334,8 +344,11 @@ __global__ void __launch_bounds__(256) k2_norm(A2Args A, u32 count) {
 #pragma unroll
       for (int q = 0; q < 3; ++q) akk[3 * r + q] = c[r] * c[q] + c[3 + r] * c[3 + q] + c[6 + r] * c[6 + q];
   }
-#pragma unroll
-  for (int r = 0; r < 9; ++r) { float t = half_sum(akk[r]); if (l16 == 0 && ok) atomicAdd(&acc[r], t); }
+  {
+    const float t = half_sum9(akk, l16);
+    const bool okh = __shfl_sync(0xffffffffu, ok, lane & 16);       // validity of the granule (its first row)
+    if (l16 < 9 && okh) atomicAdd(&acc[l16], t);
+  }
   const int ko = ok ? k : 0;
   const int kmx = max(ko, __shfl_xor_sync(0xffffffffu, ok ? k : 0, 16));
   int kw = kmx;                                                   // warp-uniform trip count (both halves, all lanes)
@@ -355,8 +368,9 @@ __global__ void __launch_bounds__(256) k2_norm(A2Args A, u32 count) {
 #pragma unroll
         for (int q = 0; q < 3; ++q) ap[3 * r + q] = cp[r] * c[q] + cp[3 + r] * c[3 + q] + cp[6 + r] * c[6 + q];
     }
-#pragma unroll
-    for (int r = 0; r < 9; ++r) { float t = half_sum(ap[r]); if (l16 == 0 && ok && p < k) atomicAdd(&acc[18 + 9 * p + r], t); }
+    const float t = half_sum9(ap, l16);
+    const int kh = __shfl_sync(0xffffffffu, ok ? k : 0, lane & 16);
+    if (l16 < 9 && p < kh) atomicAdd(&acc[18 + 9 * p + l16], t);
   }
 }
 
@@ -368,19 +382,7 @@ __global__ void __launch_bounds__(256) k2_fin(A2Args A) {
   if (s.status != 0) return;
   const float* acc = A.acc + (size_t)b * acc_stride(A.R);
   const int k = s.k;
-  float nu2 = 0.f, cross = 0.f;
-#pragma unroll
-  for (int r = 0; r < 3; ++r)
-#pragma unroll
-    for (int q = 0; q < 3; ++q) nu2 = fmaf(acc[3 * r + q], acc[9 + 3 * q + r], nu2);               // tr(A_kk B_kk)
-  for (int p = 0; p < k; ++p) {
-    const float* Ap = acc + 18 + 9 * p;
-    const float* Bp = acc + 18 + 9 * (A.R + 1) + 9 * p;
-#pragma unroll
-    for (int r = 0; r < 3; ++r)
-#pragma unroll
-      for (int q = 0; q < 3; ++q) cross = fmaf(Ap[3 * r + q], Bp[3 * q + r], cross);               // tr(A_pk B_kp)
-  }
+  const float nu2 = acc[9], cross = acc[10];
   s.lam2 += nu2 + 2.f * cross;
   s.k = k + 1;
   const float nu = sqrtf(fmaxf(nu2, 0.f)), lam = sqrtf(fmaxf(s.lam2, 0.f));
@@ -433,7 +435,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   if (chunks_pred < 1) chunks_pred = 1;
   if (chunks_pred > HH_MAX_CHUNKS) chunks_pred = HH_MAX_CHUNKS;
   // per block: table row 128 B, state 64 B, arg-max keys 32 B, P^-1 72 B, accumulators, 2 counters, 2 granules of slack
-  const size_t acc_floats = 18 + 18 * (size_t)(R + 1);
+  const size_t acc_floats = 18 + 9 * (size_t)(R + 1);
   const size_t per_block_bytes = 128 + 64 + 32 + 72 + 4 * acc_floats + 8 + 32 + 16;
   const u32 per_block_units = (u32)((per_block_bytes + 127) / 128);
   const u64 total_units = ctx->scratch_bytes / 128;

@@ -7,10 +7,11 @@
 // near-field kernel (hh_mlp.cuh).  A 2^19-row top-level block and a 20-row leaf block cost the same per entry.
 //
 // One iteration k (all blocks in lock step; blocks drop out as they stop):
-//   k_col   line 4-5  c'(i) = G(i,j_k) - sum_p C_p(i) Q_p(j_k), stored raw; arg-max scores (Eq. (9), S-18) by atomicMax
+//   k_col   line 4-5  c'(i) = G(i,j_k) - sum_p C_p(i) Q_p(j_k), stored raw; arg-max scores (Eq. (9), S-18) by atomicMax;
+//                     A'_pk = sum_i C_p(i)^T c'(i)
 //   k_piv   line 5-6  pivot row i_k, P = c'(i_k), P^-1 and cond_F(P) in fp64; zero column -> done (S-21); singular or
-//                     cond_F > kappa_max -> breakdown, block goes dense (S-18, S-18b)
-//   k_norm  line 6    c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk, A_pk = sum_i C_p(i)^T c_k(i)   (S-19)
+//                     cond_F > kappa_max -> breakdown, block goes dense (S-18, S-18b); A_pk = A'_pk P^-1
+//   k_norm  line 6    c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk = sum_i c_k(i)^T c_k(i)   (S-19)
 //   k_row   line 7-8  q_k(j) = G(i_k,j) - sum_p C_p(i_k) Q_p(j), stored raw; arg-max for j_{k+1};
 //                     nu^2 = sum_j tr(A_kk q q^T), cross = sum_j tr([sum_p Q_p(j)^T A_pk] q(j))  (= sum_p tr(A_pk B_kp), S-19)
 //   k_fin   line 9-12 lambda^2 += nu^2 + 2 cross; stop test Eq. (10) (S-20);
@@ -192,7 +193,11 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
       const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
       const int k = kk[e];
       float* acc = A.acc + (size_t)bb[e] * acc_stride(A.R);
-      // residual: subtract sum_p C_p(row) Q_p(col); the fixed operand is a broadcast load
+      // residual: subtract sum_p C_p(row) Q_p(col); the fixed operand is a broadcast load.  On the row side the same
+      // pass over the stored rows Q_p(j) also builds Z(j) = sum_p Q_p(j)^T A_pk for the cross term (S-19).
+      float Z[9];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) Z[r] = 0.f;
       for (int p = 0; p < k; ++p) {
         const float* base = chunk_ptr(A, tabrow[e], p);
         const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
@@ -205,6 +210,13 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
             qp[r] = Qp[(size_t)r * np + (COLS ? idx[e] : (u32)s.jk)];
           }
           submul33(v[e], cp, qp);
+          if (COLS) {
+            const float* Ap = acc + 18 + 9 * p;
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int c = 0; c < 3; ++c) Z[3 * r + c] += qp[r] * Ap[c] + qp[3 + r] * Ap[3 + c] + qp[6 + r] * Ap[6 + c];
+          }
         }
       }
       if (!ok[e]) {
@@ -234,25 +246,14 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
         atomicMax(&A.amax[(size_t)bb[e] * 4 + (COLS ? 3 : 1)], kf);
       }
       if (COLS) {
-        // norm recursion (S-19) with the column-side Gram matrices of k2_norm, which ran before this kernel:
-        //   nu^2 = sum_j tr(A_kk q q^T),  cross = sum_p tr(A_pk B_kp) = sum_j tr( [sum_p Q_p(j)^T A_pk] q(j) )
+        // norm recursion (S-19) with the column-side Gram matrices A_kk (k2_norm) and A_pk (k2_eval<false> + k2_piv):
+        //   nu^2 = sum_j tr(A_kk q q^T),  cross = sum_p tr(A_pk B_kp) = sum_j tr(Z(j) q(j))
         float nu2 = 0.f, cross = 0.f;
         if (ok[e]) {
-          float W[9], Z[9];
+          float W[9];
           mul33(acc, v[e], W);
 #pragma unroll
-          for (int r = 0; r < 9; ++r) { nu2 = fmaf(W[r], v[e][r], nu2); Z[r] = 0.f; }
-          for (int p = 0; p < k; ++p) {
-            const float* Qp = chunk_ptr(A, tabrow[e], p) + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
-            const float* Ap = acc + 18 + 9 * p;
-            float qp[9];
-#pragma unroll
-            for (int r = 0; r < 9; ++r) qp[r] = Qp[(size_t)r * np + idx[e]];
-#pragma unroll
-            for (int r = 0; r < 3; ++r)
-#pragma unroll
-              for (int c = 0; c < 3; ++c) Z[3 * r + c] += qp[r] * Ap[c] + qp[3 + r] * Ap[3 + c] + qp[6 + r] * Ap[6 + c];
-          }
+          for (int r = 0; r < 9; ++r) nu2 = fmaf(W[r], v[e][r], nu2);
 #pragma unroll
           for (int r = 0; r < 3; ++r)
 #pragma unroll
@@ -260,6 +261,30 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
         }
         nu2 = half_sum(nu2); cross = half_sum(cross);
         if (l16 == 0 && ok[e]) { atomicAdd(&acc[9], nu2); atomicAdd(&acc[10], cross); }
+      } else {
+        // Gram matrices of the raw column, A'_pk = sum_i C_p(i)^T c'(i); k2_piv turns them into A_pk = A'_pk P^-1.
+        // The stored columns were read a moment ago by this same thread (L1 / L2 hits, no second trip to HBM).
+        int kw = ok[e] ? k : 0;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
+        const int kh = __shfl_sync(0xffffffffu, ok[e] ? k : 0, lane & 16);
+        for (int p = 0; p < kw; ++p) {
+          float ap[9];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) ap[r] = 0.f;
+          if (ok[e] && p < k) {
+            const float* Cp = chunk_ptr(A, tabrow[e], p) + (size_t)(p % HH_RC) * 9 * mp;
+            float cp[9];
+#pragma unroll
+            for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + idx[e]];
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int c = 0; c < 3; ++c) ap[3 * r + c] = cp[r] * v[e][c] + cp[3 + r] * v[e][3 + c] + cp[6 + r] * v[e][6 + c];
+          }
+          const float t = half_sum9(ap, l16);
+          if (l16 < 9 && p < kh) atomicAdd(&acc[18 + 9 * p + l16], t);
+        }
       }
     }
   }
@@ -307,6 +332,18 @@ __global__ void __launch_bounds__(256) k2_piv(A2Args A) {
   if (sing) { a2_finish(A, b, s, 2, 2); A.st[b] = s; return; }     // S-18 / S-18b: breakdown -> the block is applied densely
 #pragma unroll
   for (int r = 0; r < 9; ++r) A.pinv[(size_t)b * 9 + r] = Pi[r];
+  // c_k = c' P^-1  =>  A_pk = sum_i C_p(i)^T c_k(i) = A'_pk P^-1
+  float* acc = A.acc + (size_t)b * acc_stride(A.R);
+  for (int p = 0; p < s.k; ++p) {
+    float* Ap = acc + 18 + 9 * p;
+    double a[9];
+#pragma unroll
+    for (int r = 0; r < 9; ++r) a[r] = (double)Ap[r];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int q = 0; q < 3; ++q) Ap[3 * r + q] = (float)(a[3 * r] * Pi[q] + a[3 * r + 1] * Pi[3 + q] + a[3 * r + 2] * Pi[6 + q]);
+  }
   s.ik = ik;
   A.st[b] = s;
 }
@@ -348,29 +385,6 @@ __global__ void __launch_bounds__(256) k2_norm(A2Args A, u32 count) {
     const float t = half_sum9(akk, l16);
     const bool okh = __shfl_sync(0xffffffffu, ok, lane & 16);       // validity of the granule (its first row)
     if (l16 < 9 && okh) atomicAdd(&acc[l16], t);
-  }
-  const int ko = ok ? k : 0;
-  const int kmx = max(ko, __shfl_xor_sync(0xffffffffu, ok ? k : 0, 16));
-  int kw = kmx;                                                   // warp-uniform trip count (both halves, all lanes)
-#pragma unroll
-  for (int o = 8; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
-  for (int p = 0; p < kw; ++p) {
-    float ap[9];
-#pragma unroll
-    for (int r = 0; r < 9; ++r) ap[r] = 0.f;
-    if (ok && p < k) {
-      const float* Cp = chunk_ptr(A, tabrow, p) + (size_t)(p % HH_RC) * 9 * mp;
-      float cp[9];
-#pragma unroll
-      for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + i];
-#pragma unroll
-      for (int r = 0; r < 3; ++r)
-#pragma unroll
-        for (int q = 0; q < 3; ++q) ap[3 * r + q] = cp[r] * c[q] + cp[3 + r] * c[3 + q] + cp[6 + r] * c[6 + q];
-    }
-    const float t = half_sum9(ap, l16);
-    const int kh = __shfl_sync(0xffffffffu, ok ? k : 0, lane & 16);
-    if (l16 < 9 && p < kh) atomicAdd(&acc[18 + 9 * p + l16], t);
   }
 }
 

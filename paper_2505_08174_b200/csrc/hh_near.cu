@@ -8,7 +8,7 @@
 #define NR_T 256
 #define NR_TILE 512
 
-__global__ void __launch_bounds__(NR_T) k_near(const float* __restrict__ gw, float a, const u32* __restrict__ leaf_nodes,
+__global__ void __launch_bounds__(NR_T, 2) k_near(const float* __restrict__ gw, float a, const u32* __restrict__ leaf_nodes,
                                                 const u32* __restrict__ nlo, const u32* __restrict__ nhi,
                                                 const uint2* __restrict__ PH, const u32* __restrict__ near_begin,
                                                 const u32* __restrict__ near_end, const float* __restrict__ Xs,

@@ -30,7 +30,7 @@ if ROOT not in sys.path:
 METRIC = "H-matvec particles/s (whole step: tree + blocks + ACA + near + far + three-body)"
 UNIT = "particles/s"
 FAR_BYTES_PER_UNIT = 36          # bytes of fp32 factors read per (row or column) x block-rank (DESIGN.md far-field)
-ORACLE_SAMPLE_N = {"c1": 2048, "c2": 4096, "c3": 8192, "c4": 8192, "c5": 8000}
+ORACLE_SAMPLE_N = {"c1": 2048, "c2": 8192, "c3": 24576, "c4": 16384, "c5": 16000}
 
 
 def peaks():

@@ -72,6 +72,8 @@ typedef struct {
   float   kappa_max;     /* S-18b: a pivot block with |P|_F |P^-1|_F above this is numerically singular at fp32
                             entry accuracy: Alg. 2 breaks down on that block (flag 2) and the mat-vec evaluates it
                             densely like an inadmissible block (L252).  0 = default (300); INFINITY = never   */
+  float   dense_cap;     /* S-18b applies where the dense evaluation is affordable: |tau||sigma| <= dense_cap (|tau|+|sigma|);
+                            larger blocks keep the ill-conditioned pivot (plain listing).  0 = default (128)          */
 } hh_params;
 
 /* Counters (Figs. 7-9 count "queries" = MLP evaluations; L299). Filled as stages run. */

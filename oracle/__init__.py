@@ -152,6 +152,10 @@ class HMatrix:
         densely).  Default 300; float('inf') gives the plain listing."""
         lib().orc_h_set_kappa_max(self._h, C.c_double(kappa))
 
+    def set_dense_cap(self, cap):
+        """S-18b applies to blocks with |tau||sigma| <= cap (|tau| + |sigma|) only (default 128)."""
+        lib().orc_h_set_dense_cap(self._h, C.c_double(cap))
+
     def last_bad_strict(self):
         """slack-only count of bad decisions of the last replay call (reported, not asserted)"""
         return int(lib().orc_h_last_bad_strict(self._h))

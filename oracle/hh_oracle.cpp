@@ -380,7 +380,8 @@ int argmax_score(const std::vector<double>& v, int n, const std::vector<char>& u
 // decisions that are not an arg-max / a correct stop within `slack` (relative).
 void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t snode, double zeta,
                int max_rank, int rule, int rp_rank, const int32_t* rp_i, const int32_t* rp_j,
-               double slack, AcaOut& out, double u_round = 0.0, double kappa_max = 300.0, int rp_flag = 0) {
+               double slack, AcaOut& out, double u_round = 0.0, double kappa_max = 300.0, int rp_flag = 0,
+               double dense_cap = 128.0) {
   const Node& T = h.nodes[tnode];
   const Node& S = h.nodes[snode];
   int c = (int)(T.hi - T.lo), q = (int)(S.hi - S.lo);
@@ -391,6 +392,9 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
   // a replayed run that broke down (flag 2) lists rp_rank accepted pivots plus the attempted one
   const int rp_len = replay ? rp_rank + (rp_flag == 2 ? 1 : 0) : 0;
   if (replay) kmax = std::min(kmax, rp_len);
+  // S-18b applies where the dense evaluation is affordable: |tau||sigma| <= dense_cap (|tau| + |sigma|); a larger
+  // block keeps the ill-conditioned pivot, as the plain listing does
+  const bool dense_ok = (double)c * (double)q <= dense_cap * ((double)c + (double)q);
   std::vector<char> used_r(c, 0), used_c(q, 0);
   std::vector<double> ck((size_t)9 * c), qk((size_t)9 * q);
   std::vector<double> errc(c, 0.0), errq(q, 0.0), kappa;        // replay-mode rounding bounds (checker only)
@@ -448,7 +452,7 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     }
     inv33(P, dP, Pinv);
     const double kap = std::sqrt(fro2(P) * fro2(Pinv)), pinv_n = std::sqrt(fro2(Pinv));
-    if (!replay && kap > kappa_max) {                            // S-18b: numerically singular pivot
+    if (!replay && dense_ok && kap > kappa_max) {                // S-18b: numerically singular pivot
       out.flag = 2;
       out.piv_i.push_back(ik); out.piv_j.push_back(jk);
       break;
@@ -458,12 +462,12 @@ void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t s
     const double e_piv = errc[ik] * pinv_n;
     const double kap_lo = kap / (1.0 + e_piv), kap_hi = e_piv < 1.0 ? kap / (1.0 - e_piv) : INFINITY;
     if (attempted) {                                             // replay: the breakdown must be plausible (factor 2 on cond)
-      if (kap < 0.5 * kappa_max) { out.replay_bad_strict++; if (kap_hi < 0.5 * kappa_max) out.replay_bad++; }
+      if (kap < 0.5 * kappa_max || !dense_ok) { out.replay_bad_strict++; if (kap_hi < 0.5 * kappa_max || !dense_ok) out.replay_bad++; }
       out.flag = 2;
       out.piv_i.push_back(ik); out.piv_j.push_back(jk);
       break;
     }
-    if (replay && kap > 2.0 * kappa_max) {                       // should have broken down here
+    if (replay && dense_ok && kap > 2.0 * kappa_max) {           // should have broken down here
       out.replay_bad_strict++;
       if (kap_lo > 2.0 * kappa_max) out.replay_bad++;
     }
@@ -592,6 +596,7 @@ struct Handle {
   double a = 1.0;
   double u_round = 0.0;         // replay checker: unit roundoff of the replayed arithmetic (0 = slack only)
   double kappa_max = 300.0;     // S-18b: pivot blocks with cond_F above this break Alg. 2 down (block goes dense)
+  double dense_cap = 128.0;     // S-18b only where |tau||sigma| <= dense_cap (|tau| + |sigma|)
   int64_t last_bad_strict = 0;  // slack-only count of the last replay call
 };
 
@@ -748,6 +753,7 @@ void orc_h_destroy(void* p) { delete (Handle*)p; }
 // replay checker: unit roundoff of the arithmetic being replayed (2^-24 for the fp32 CUDA path; 0 = slack only)
 void orc_h_set_replay_roundoff(void* p, double u) { ((Handle*)p)->u_round = u; }
 void orc_h_set_kappa_max(void* p, double k) { ((Handle*)p)->kappa_max = k; }
+void orc_h_set_dense_cap(void* p, double c) { ((Handle*)p)->dense_cap = c; }
 int64_t orc_h_last_bad_strict(void* p) { return ((Handle*)p)->last_bad_strict; }
 
 void orc_h_counts(void* p, int64_t* n_nodes, int64_t* n_leaves, int64_t* nG, int64_t* nH, int64_t* depth) {
@@ -793,7 +799,7 @@ int orc_h_aca_block(void* p, int64_t gblock, double zeta, int max_rank, int rule
   auto pr = H->h.G[(size_t)gblock];
   AcaOut o;
   aca_block(H->h, H->mlp2, H->a, pr.first, pr.second, zeta, max_rank, rule, rp_rank, rp_i, rp_j, slack, o, H->u_round,
-            H->kappa_max, rp_flag);
+            H->kappa_max, rp_flag, H->dense_cap);
   H->last_bad_strict = o.replay_bad_strict;
   int c = (int)(H->h.nodes[pr.first].hi - H->h.nodes[pr.first].lo);
   int q = (int)(H->h.nodes[pr.second].hi - H->h.nodes[pr.second].lo);
@@ -883,10 +889,11 @@ int64_t orc_h_matvec(void* p, const float* F, double zeta, int max_rank, int rul
       AcaOut o;
       if (rp_rank)
         aca_block(h, Hd->mlp2, Hd->a, h.G[g].first, h.G[g].second, zeta, max_rank, rule, rp_rank[g],
-                  rp_i + rp_off[g], rp_j + rp_off[g], slack, o, Hd->u_round, Hd->kappa_max, rp_flag ? rp_flag[g] : 0);
+                  rp_i + rp_off[g], rp_j + rp_off[g], slack, o, Hd->u_round, Hd->kappa_max, rp_flag ? rp_flag[g] : 0,
+                  Hd->dense_cap);
       else
         aca_block(h, Hd->mlp2, Hd->a, h.G[g].first, h.G[g].second, zeta, max_rank, rule, -1, nullptr, nullptr, 0.0, o, 0.0,
-                  Hd->kappa_max, 0);
+                  Hd->kappa_max, 0, Hd->dense_cap);
       entries += (int64_t)o.rank * (c + q);
       bad += o.replay_bad;
       bad_strict += o.replay_bad_strict;

@@ -12,7 +12,7 @@
 #include "hh_mlp.cuh"
 
 struct AcaArgs {
-  const float* w2; float a; float tol; int max_rank; int rule; double kappa_max;
+  const float* w2; float a; float tol; int max_rank; int rule; double kappa_max, dense_cap;
   const uint2* PG; const u32 *nlo, *nhi; const float* Xs;
   float* arena; u64 arena_units; u32* tab; DevScalars* sc;
   int *ranks, *flags;
@@ -193,7 +193,8 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 384 / T) k_aca(AcaArgs A) {
         double np2 = 0.0, ni2 = 0.0;
 #pragma unroll
         for (int r = 0; r < 9; ++r) { np2 += P[r] * P[r]; ni2 += S.sPinvD[r] * S.sPinvD[r]; }
-        if (sqrt(np2 * ni2) > A.kappa_max) S.ctl[1] = 2;          // S-18b: numerically singular at fp32 entry accuracy
+        if (sqrt(np2 * ni2) > A.kappa_max && (double)m * (double)n <= A.dense_cap * ((double)m + (double)n))
+          S.ctl[1] = 2;                                           // S-18b: numerically singular at fp32 entry accuracy
       }
       S.piv_i[k] = ik;
     }
@@ -427,6 +428,7 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   AcaArgs A;
   A.w2 = ctx->w2; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.max_rank = ctx->p.aca_max_rank; A.rule = ctx->p.pivot_rule;
   A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : 300.0;
+  A.dense_cap = ctx->p.dense_cap > 0.f ? (double)ctx->p.dense_cap : 128.0;
   A.PG = ctx->PG; A.nlo = ctx->nlo; A.nhi = ctx->nhi; A.Xs = ctx->Xs;
   A.arena = ctx->arena; A.arena_units = ctx->arena_units; A.tab = ctx->tab; A.sc = ctx->d_sc;
   A.ranks = ctx->ranks; A.flags = ctx->flags; A.first = (u32)first;

@@ -34,7 +34,7 @@ struct BlkState {                /* 64 bytes per block of the batch             
 };
 
 struct A2Args {
-  const float* w2; float a; float tol; int rule; double kappa_max;
+  const float* w2; float a; float tol; int rule; double kappa_max, dense_cap;
   const uint2* PG; const u32 *nlo, *nhi; const float* Xs;
   float* arena; u64 arena_units; u32* tab; DevScalars* sc;
   int *ranks, *flags;
@@ -327,7 +327,8 @@ __global__ void __launch_bounds__(256) k2_piv(A2Args A) {
     double np2 = 0.0, ni2 = 0.0;
 #pragma unroll
     for (int r = 0; r < 9; ++r) { np2 += P[r] * P[r]; ni2 += Pi[r] * Pi[r]; }
-    sing = sqrt(np2 * ni2) > A.kappa_max;                          // S-18b
+    sing = sqrt(np2 * ni2) > A.kappa_max &&                        // S-18b, where the dense evaluation is affordable
+           (double)s.m * (double)s.n <= A.dense_cap * ((double)s.m + (double)s.n);
   }
   if (sing) { a2_finish(A, b, s, 2, 2); A.st[b] = s; return; }     // S-18 / S-18b: breakdown -> the block is applied densely
 #pragma unroll
@@ -483,6 +484,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     ctx->arena_units = (ctx->scratch_bytes - off) / 128;
     A.w2 = ctx->w2; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.rule = ctx->p.pivot_rule;
     A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : 300.0;
+    A.dense_cap = ctx->p.dense_cap > 0.f ? (double)ctx->p.dense_cap : 128.0;
     A.PG = ctx->PG; A.nlo = ctx->nlo; A.nhi = ctx->nhi; A.Xs = ctx->Xs;
     A.arena = ctx->arena; A.arena_units = ctx->arena_units; A.tab = ctx->tab; A.sc = ctx->d_sc;
     A.ranks = ctx->ranks; A.flags = ctx->flags; A.first = (u32)first; A.nb = nb; A.R = R;

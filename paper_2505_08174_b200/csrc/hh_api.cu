@@ -70,7 +70,8 @@ static int check_params(const hh_params* p) {
   if (!(p->rcut3 >= 0.f) || !isfinite(p->rcut3)) return 0;
   if (p->pivot_rule != 0 && p->pivot_rule != 1) return 0;
   if (p->near_path != 0) return 0;
-  if (!(p->kappa_max >= 0.f)) return 0;                           /* 0 = default, INFINITY allowed, NaN / negative not */
+  if (!(p->kappa_max >= 0.f)) return 0;
+  if (!(p->dense_cap >= 0.f)) return 0;                           /* 0 = default, INFINITY allowed, NaN / negative not */
   return 1;
 }
 

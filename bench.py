@@ -89,6 +89,17 @@ class ClockSampler:
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def max_over_ranks(value, world, device):
+    """max of a per-rank scalar over all ranks (the contract's max-over-ranks timing); no data-path collective exists"""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def make_inputs(workload, rank):
     """seeded synthetic cloud of the named config; replicas (rank > 0) draw their own seed"""
     import synth
@@ -231,10 +242,7 @@ def run_gpu(args):
     t_wall = time.perf_counter() - t_wall
     clk = clocks.stop() if rank == 0 else None
     total_ms = float(sum(ms))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, dev)
     assert torch.isfinite(Ud).all().item(), "non-finite velocities"
 
     # ---- end to end through the public API with HOST buffers (pinned), copies inside the timed region ----
@@ -250,10 +258,7 @@ def run_gpu(args):
         ctx.step_host(Xh, Fh, Uh, dt=dt)                                # returns after the D2H copies have completed
     torch.cuda.synchronize(dev)
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = max_over_ranks(e2e_s, world, dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

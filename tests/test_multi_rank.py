@@ -21,7 +21,7 @@ local_ms = 100.0 + 50.0 * rank                       # rank 1 is the slow one
 mx = bench.max_over_ranks(local_ms, world, torch.device("cpu"))
 cfg, X, F = bench.make_inputs("c1", rank)
 dist.barrier()
-open(os.path.join(os.environ["HH_TEST_OUT"], "rank%d.json" % rank), "w").write(
+open(os.path.join(os.environ["HH_TEST_OUT"], "rank%%d.json" %% rank), "w").write(
     json.dumps({"rank": rank, "world": world, "max": mx, "x0": float(X[0, 0]), "f0": float(F[0, 0]), "n": len(X)}))
 dist.destroy_process_group()
 """ % ROOT

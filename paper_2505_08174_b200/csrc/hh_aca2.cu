@@ -7,6 +7,7 @@
 // near-field kernel (hh_mlp.cuh).  A 2^19-row top-level block and a 20-row leaf block cost the same per entry.
 //
 // One iteration k (all blocks in lock step; blocks drop out as they stop):
+//   (each of k_col / k_row is two launches: k2_mlp evaluates and stores the raw entries, k2_upd does the rest)
 //   k_col   line 4-5  c'(i) = G(i,j_k) - sum_p C_p(i) Q_p(j_k), stored raw; arg-max scores (Eq. (9), S-18) by atomicMax;
 //                     A'_pk = sum_i C_p(i)^T c'(i)
 //   k_piv   line 5-6  pivot row i_k, P = c'(i_k), P^-1 and cond_F(P) in fp64; zero column -> done (S-21); singular or
@@ -152,10 +153,13 @@ __global__ void __launch_bounds__(256) k2_gran_fill(A2Args A) {                /
   for (u32 t = lane; t < nn; t += 32) A.gn[pn + t] = make_uint2(b, t * GR);
 }
 
-// ---- lines 4-5 (COLS = false: over the rows of tau) and lines 7-8 (COLS = true: over the columns of sigma) ----
+// ---- lines 4 and 7, first half: the entries G(i, j_k) (COLS = false: over the rows of tau) resp. G(i_k, j) (COLS = true:
+// over the columns of sigma) of all active blocks, evaluated by the MLP and stored raw in the slot of rank k.
 // A warp takes 4 granules: slot (e, half) -> granule 4*tile + 2*e + half; every thread evaluates two entries.
+// Nothing else happens here, so this kernel runs at the speed of the near-field kernel; the residual, the pivot
+// scores and the Gram sums are the bandwidth-bound second half (k2_upd), which runs at four times the occupancy.
 template <bool COLS>
-__global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
+__global__ void __launch_bounds__(A2_T, 2) k2_mlp(A2Args A, u32 count) {
   __shared__ __align__(16) float sw[HH_MLP2_FLOATS];
   load_weights(sw, A.w2, HH_MLP2_FLOATS);
   __syncthreads();
@@ -163,129 +167,144 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
   const uint2* gl = COLS ? A.gn : A.gm;
   const u32 ntiles = (count + 3) / 4;
   for (u32 tile = blockIdx.x * (A2_T / 32) + warp; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
-    u32 bb[2], idx[2], len[2], lenp[2];
-    int kk[2];
-    bool ok[2];
+    u32 idx[2], len[2], lenp[2];
+    bool ok[2], live[2];
     float xi[2][3], xj[2][3], v[2][9];
-    const u32* tabrow[2];
+    float* dst[2];
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const u32 gi = 4 * tile + 2 * e + half;
       const bool gv = gi < count;
       const uint2 g = gl[gv ? gi : count - 1];
-      bb[e] = g.x; idx[e] = g.y + l16;
+      idx[e] = g.y + l16;
       const BlkState& s = A.st[g.x];
+      const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
       len[e] = COLS ? s.n : s.m;
-      lenp[e] = a2_pad8(len[e]);
-      kk[e] = s.k;
-      ok[e] = gv && s.status == 0 && idx[e] < len[e];
-      tabrow[e] = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+      lenp[e] = COLS ? np : mp;
+      live[e] = gv && s.status == 0;
+      ok[e] = live[e] && idx[e] < len[e];
+      const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+      dst[e] = chunk_ptr(A, tabrow, s.k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(s.k % HH_RC) * 9 * np : (size_t)(s.k % HH_RC) * 9 * mp);
       const u32 ic = idx[e] < len[e] ? idx[e] : len[e] - 1;
       const u32 ti = COLS ? s.tlo + (u32)(s.ik < 0 ? 0 : s.ik) : s.tlo + ic;   // target (row) particle (ik unset on blocks that just stopped)
-      const u32 sj = COLS ? s.slo + ic : s.slo + (u32)s.jk;            // source (column) particle
+      const u32 sj = COLS ? s.slo + ic : s.slo + (u32)s.jk;                    // source (column) particle
 #pragma unroll
       for (int d = 0; d < 3; ++d) { xi[e][d] = A.Xs[3 * (size_t)ti + d]; xj[e][d] = A.Xs[3 * (size_t)sj + d]; }
     }
     entry2_eval<2>(sw, A.a, xi, xj, v);
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
-      const BlkState& s = A.st[bb[e]];
-      const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
-      const int k = kk[e];
-      float* acc = A.acc + (size_t)bb[e] * acc_stride(A.R);
-      // residual: subtract sum_p C_p(row) Q_p(col); the fixed operand is a broadcast load.  On the row side the same
-      // pass over the stored rows Q_p(j) also builds Z(j) = sum_p Q_p(j)^T A_pk for the cross term (S-19).
-      float Z[9];
-#pragma unroll
-      for (int r = 0; r < 9; ++r) Z[r] = 0.f;
-      for (int p = 0; p < k; ++p) {
-        const float* base = chunk_ptr(A, tabrow[e], p);
-        const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
-        const float* Qp = base + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
-        float cp[9], qp[9];
-        if (ok[e]) {
-#pragma unroll
-          for (int r = 0; r < 9; ++r) {
-            cp[r] = Cp[(size_t)r * mp + (COLS ? (u32)s.ik : idx[e])];
-            qp[r] = Qp[(size_t)r * np + (COLS ? idx[e] : (u32)s.jk)];
-          }
-          submul33(v[e], cp, qp);
-          if (COLS) {
-            const float* Ap = acc + 18 + 9 * p;
-#pragma unroll
-            for (int r = 0; r < 3; ++r)
-#pragma unroll
-              for (int c = 0; c < 3; ++c) Z[3 * r + c] += qp[r] * Ap[c] + qp[3 + r] * Ap[3 + c] + qp[6 + r] * Ap[6 + c];
-          }
-        }
-      }
-      if (!ok[e]) {
-#pragma unroll
-        for (int r = 0; r < 9; ++r) v[e][r] = 0.f;
-      }
-      // store the raw residual (column: normalised later by k2_norm; row: kept raw, listing line 7)
-      float* dst = chunk_ptr(A, tabrow[e], k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np : (size_t)(k % HH_RC) * 9 * mp);
       if (ok[e]) {
 #pragma unroll
-        for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp[e] + idx[e]] = v[e][r];
-      } else if (COLS && 4 * tile + 2 * e + half < count && s.status == 0 && idx[e] < lenp[e]) {
+        for (int r = 0; r < 9; ++r) dst[e][(size_t)r * lenp[e] + idx[e]] = v[e][r];
+      } else if (COLS && live[e] && idx[e] < lenp[e]) {
 #pragma unroll
-        for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp[e] + idx[e]] = 0.f;        // zero the pad columns (far kernel reads float4)
+        for (int r = 0; r < 9; ++r) dst[e][(size_t)r * lenp[e] + idx[e]] = 0.f;      // zero the pad columns (far kernel reads float4)
       }
-      // arg-max scores over unused rows / columns (Eq. (9); S-18)
-      unsigned long long kd = 0ull, kf = 0ull;
-      if (ok[e]) {
-        const int* piv = a2_piv(A, bb[e]) + (COLS ? HH_MAX_RANK : 0);
-        bool used = false;
-        for (int q = 0; q < k + (COLS ? 1 : 0); ++q) used |= (piv[q] == (int)idx[e]);
-        if (!used) { kd = amax_key(fabsf(det33(v[e])), idx[e]); kf = amax_key(fro2_33(v[e]), idx[e]); }
+    }
+  }
+}
+
+// ---- lines 4-5 resp. 7-8, second half: residual against the stored rank terms, pivot scores, Gram sums.
+// Half a warp per granule, one entry per thread.
+template <bool COLS>
+__global__ void __launch_bounds__(256, 4) k2_upd(A2Args A, u32 count) {
+  const u32 lane = threadIdx.x & 31, l16 = lane & 15;
+  const u32 gi = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
+  const bool gv = gi < count;
+  const uint2 g = (COLS ? A.gn : A.gm)[gv ? gi : count - 1];
+  const BlkState& s = A.st[g.x];
+  const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
+  const u32 len = COLS ? s.n : s.m, lenp = COLS ? np : mp, idx = g.y + l16;
+  const int k = s.k;
+  const bool ok = gv && s.status == 0 && idx < len;
+  const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+  float* acc = A.acc + (size_t)g.x * acc_stride(A.R);
+  float* dst = chunk_ptr(A, tabrow, k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np : (size_t)(k % HH_RC) * 9 * mp);
+  float v[9], Z[9];
+#pragma unroll
+  for (int r = 0; r < 9; ++r) { v[r] = ok ? dst[(size_t)r * lenp + idx] : 0.f; Z[r] = 0.f; }
+  // residual: subtract sum_p C_p(row) Q_p(col); the fixed operand is a broadcast load.  On the row side the same pass
+  // over the stored rows Q_p(j) also builds Z(j) = sum_p Q_p(j)^T A_pk for the cross term (S-19).
+  if (ok) {
+    const u32 fix = COLS ? (u32)s.ik : (u32)s.jk;
+#pragma unroll 2
+    for (int p = 0; p < k; ++p) {
+      const float* base = chunk_ptr(A, tabrow, p);
+      const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
+      const float* Qp = base + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
+      float cp[9], qp[9];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) {
+        cp[r] = Cp[(size_t)r * mp + (COLS ? fix : idx)];
+        qp[r] = Qp[(size_t)r * np + (COLS ? idx : fix)];
       }
-      kd = half_max(kd); kf = half_max(kf);
-      if (l16 == 0 && (kd | kf)) {
-        atomicMax(&A.amax[(size_t)bb[e] * 4 + (COLS ? 2 : 0)], kd);
-        atomicMax(&A.amax[(size_t)bb[e] * 4 + (COLS ? 3 : 1)], kf);
-      }
+      submul33(v, cp, qp);
       if (COLS) {
-        // norm recursion (S-19) with the column-side Gram matrices A_kk (k2_norm) and A_pk (k2_eval<false> + k2_piv):
-        //   nu^2 = sum_j tr(A_kk q q^T),  cross = sum_p tr(A_pk B_kp) = sum_j tr(Z(j) q(j))
-        float nu2 = 0.f, cross = 0.f;
-        if (ok[e]) {
-          float W[9];
-          mul33(acc, v[e], W);
+        const float* Ap = acc + 18 + 9 * p;
 #pragma unroll
-          for (int r = 0; r < 9; ++r) nu2 = fmaf(W[r], v[e][r], nu2);
+        for (int r = 0; r < 3; ++r)
 #pragma unroll
-          for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) cross = fmaf(Z[3 * r + c], v[e][3 * c + r], cross);
-        }
-        nu2 = half_sum(nu2); cross = half_sum(cross);
-        if (l16 == 0 && ok[e]) { atomicAdd(&acc[9], nu2); atomicAdd(&acc[10], cross); }
-      } else {
-        // Gram matrices of the raw column, A'_pk = sum_i C_p(i)^T c'(i); k2_piv turns them into A_pk = A'_pk P^-1.
-        // The stored columns were read a moment ago by this same thread (L1 / L2 hits, no second trip to HBM).
-        int kw = ok[e] ? k : 0;
-#pragma unroll
-        for (int o = 16; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
-        const int kh = __shfl_sync(0xffffffffu, ok[e] ? k : 0, lane & 16);
-        for (int p = 0; p < kw; ++p) {
-          float ap[9];
-#pragma unroll
-          for (int r = 0; r < 9; ++r) ap[r] = 0.f;
-          if (ok[e] && p < k) {
-            const float* Cp = chunk_ptr(A, tabrow[e], p) + (size_t)(p % HH_RC) * 9 * mp;
-            float cp[9];
-#pragma unroll
-            for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + idx[e]];
-#pragma unroll
-            for (int r = 0; r < 3; ++r)
-#pragma unroll
-              for (int c = 0; c < 3; ++c) ap[3 * r + c] = cp[r] * v[e][c] + cp[3 + r] * v[e][3 + c] + cp[6 + r] * v[e][6 + c];
-          }
-          const float t = half_sum9(ap, l16);
-          if (l16 < 9 && p < kh) atomicAdd(&acc[18 + 9 * p + l16], t);
-        }
+          for (int c = 0; c < 3; ++c) Z[3 * r + c] += qp[r] * Ap[c] + qp[3 + r] * Ap[3 + c] + qp[6 + r] * Ap[6 + c];
       }
+    }
+    if (k > 0) {
+#pragma unroll
+      for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp + idx] = v[r];   // the residual (column: normalised later by k2_norm; row: kept raw)
+    }
+  }
+  // arg-max scores over unused rows / columns (Eq. (9); S-18)
+  unsigned long long kd = 0ull, kf = 0ull;
+  if (ok) {
+    const int* piv = a2_piv(A, g.x) + (COLS ? HH_MAX_RANK : 0);
+    bool used = false;
+    for (int q = 0; q < k + (COLS ? 1 : 0); ++q) used |= (piv[q] == (int)idx);
+    if (!used) { kd = amax_key(fabsf(det33(v)), idx); kf = amax_key(fro2_33(v), idx); }
+  }
+  kd = half_max(kd); kf = half_max(kf);
+  if (l16 == 0 && (kd | kf)) {
+    atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 2 : 0)], kd);
+    atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 3 : 1)], kf);
+  }
+  if (COLS) {
+    // norm recursion (S-19) with the column-side Gram matrices A_kk (k2_norm) and A_pk (k2_upd<false> + k2_piv):
+    //   nu^2 = sum_j tr(A_kk q q^T),  cross = sum_p tr(A_pk B_kp) = sum_j tr(Z(j) q(j))
+    float nu2 = 0.f, cross = 0.f;
+    if (ok) {
+      float W[9];
+      mul33(acc, v, W);
+#pragma unroll
+      for (int r = 0; r < 9; ++r) nu2 = fmaf(W[r], v[r], nu2);
+#pragma unroll
+      for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int c = 0; c < 3; ++c) cross = fmaf(Z[3 * r + c], v[3 * c + r], cross);
+    }
+    nu2 = half_sum(nu2); cross = half_sum(cross);
+    if (l16 == 0 && ok) { atomicAdd(&acc[9], nu2); atomicAdd(&acc[10], cross); }
+  } else {
+    // Gram matrices of the raw column, A'_pk = sum_i C_p(i)^T c'(i); k2_piv turns them into A_pk = A'_pk P^-1.
+    // The stored columns were read a moment ago by this same thread (L1 / L2 hits, no second trip to HBM).
+    int kw = ok ? k : 0;
+#pragma unroll
+    for (int o = 16; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
+    const int kh = __shfl_sync(0xffffffffu, ok ? k : 0, lane & 16);
+    for (int p = 0; p < kw; ++p) {
+      float ap[9];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) ap[r] = 0.f;
+      if (ok && p < k) {
+        const float* Cp = chunk_ptr(A, tabrow, p) + (size_t)(p % HH_RC) * 9 * mp;
+        float cp[9];
+#pragma unroll
+        for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + idx];
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) ap[3 * r + c] = cp[r] * v[c] + cp[3 + r] * v[3 + c] + cp[6 + r] * v[6 + c];
+      }
+      const float t = half_sum9(ap, l16);
+      if (l16 < 9 && p < kh) atomicAdd(&acc[18 + 9 * p + l16], t);
     }
   }
 }
@@ -505,10 +524,12 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       k2_gran_fill<<<HH_N + cdiv((int64_t)nb * 32, 256), 256, 0, s>>>(A);
       const unsigned cap = 148 * 2 * 4;
       unsigned g1 = cdiv(cdiv(gmc, 4), A2_T / 32), g2 = cdiv(cdiv(gnc, 4), A2_T / 32);
-      k2_eval<false><<<HH_N + (g1 < cap ? g1 : cap), A2_T, 0, s>>>(A, gmc);
+      k2_mlp<false><<<HH_N + (g1 < cap ? g1 : cap), A2_T, 0, s>>>(A, gmc);
+      k2_upd<false><<<HH_N + cdiv((int64_t)gmc * GR, 256), 256, 0, s>>>(A, gmc);
       k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
       k2_norm<<<HH_N + cdiv((int64_t)gmc * GR, 256), 256, 0, s>>>(A, gmc);
-      k2_eval<true><<<HH_N + (g2 < cap ? g2 : cap), A2_T, 0, s>>>(A, gnc);
+      k2_mlp<true><<<HH_N + (g2 < cap ? g2 : cap), A2_T, 0, s>>>(A, gnc);
+      k2_upd<true><<<HH_N + cdiv((int64_t)gnc * GR, 256), 256, 0, s>>>(A, gnc);
       k2_fin<<<HH_N + gb, 256, 0, s>>>(A);
       HH_LAUNCH_CHECK();
     }

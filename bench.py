@@ -171,9 +171,9 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def workload_name(w):
+def workload_name(w, c=None):
     import synth
-    c = synth.CONFIGS[w]
+    c = c or synth.CONFIGS[w]
     return ("%s: N=%d %s phi=%.2f, leaf %d, eta=%.1f, zeta=%.0e, rcut3=%.1f, MLP2 4-32-32-9, MLP3 7-64-64-9 (BASELINE.json configs[%d])"
             % (w, c["n"], c["shape"], c["phi"], c["leaf"], c["eta"], c["tol"], c["rcut3"], int(w[1]) - 1))
 
@@ -196,13 +196,16 @@ def run_gpu(args):
         dist.init_process_group("nccl", device_id=dev)
 
     cfg, X, F = make_inputs(args.workload, rank)
+    for key, val in (("eta", args.eta), ("tol", args.tol), ("leaf", args.leaf), ("kappa_max", args.kappa_max)):
+        if val is not None:
+            cfg[key] = val                                              # sweeps of config 3 (eta, zeta); otherwise the config's own
     N = len(X)
     mlp2 = synth.xavier_mlp(synth.MLP2_DIMS, 1)
     mlp3 = synth.xavier_mlp(synth.MLP3_DIMS, 3) if cfg["rcut3"] > 0 else None
     free, _ = torch.cuda.mem_get_info(dev)
     ws = int(min(free * 0.85, args.workspace_gb * (1 << 30)))
     ctx = hh.Context(mlp2, mlp3, leaf_size=cfg["leaf"], eta=cfg["eta"], aca_tol=cfg["tol"], rcut3=cfg["rcut3"],
-                     workspace_bytes=ws, device=dev)
+                     kappa_max=float(cfg.get("kappa_max", 0.0)), workspace_bytes=ws, device=dev)
     ctx.enable_timing(True)
     stream = torch.cuda.current_stream(dev)
     Xd = torch.from_numpy(X).to(dev)
@@ -278,7 +281,7 @@ def run_gpu(args):
         "metric": METRIC, "value": world * N * K / (total_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": K,
         "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(args.workload), "parallelism": "replicas x%d (no sharding, no collectives)" % world,
+        "config": {"workload": workload_name(args.workload, cfg), "parallelism": "replicas x%d (no sharding, no collectives)" % world,
                    "l2": "explicit 256 MB flush write between timed iterations; each step also streams its factor arena (>> L2)",
                    "arena_gb": st["arena_bytes"] / 2 ** 30, "aca_batches_per_step": st["aca_batches"]},
         "clocks": clk,
@@ -316,6 +319,10 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workspace-gb", type=float, default=150.0)
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--eta", type=float, default=None, help="override the config's eta (config 3 sweep)")
+    ap.add_argument("--tol", type=float, default=None, help="override the config's ACA tolerance zeta (config 3 sweep)")
+    ap.add_argument("--leaf", type=int, default=None)
+    ap.add_argument("--kappa-max", type=float, default=None, help="S-18b limit on the pivot-block condition number")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     args = ap.parse_args()
     args.warmup_ref = min(args.warmup, 1)

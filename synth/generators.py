@@ -139,7 +139,7 @@ CONFIGS = {
     "c4": dict(n=10000000, shape="cube", phi=0.05, forces="gaussian", leaf=128, eta=1.0, tol=1e-4,
                rcut3=4.0, steps=1, dt=0.0),
     "c5": dict(n=1000000, shape="chains", phi=0.1, forces="filament", leaf=64, eta=1.0, tol=1e-4,
-               rcut3=4.0, steps=100, dt=0.005, n_chains=20000, n_beads=50),
+               rcut3=4.0, steps=100, dt=0.005, n_chains=20000, n_beads=50, kappa_max=50.0),   # S-18b: chains need 50 for the 1e-5 bar
 }
 
 

@@ -147,9 +147,10 @@ int hh_matvec(hh_ctx* ctx, const float* F, float* U);
 int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts);
 
 /* Far-field apply only, over the factors currently in the arena (blocks [first, next) of the last
- * hh_aca call): Us_tree += C (Q F^sigma).  The roofline-graded kernel.
+ * hh_aca call): Us_tree += C (Q F^sigma), the roofline-graded kernel; resident
+ * blocks on which Alg. 2 broke down (flag 2, S-18b) are added densely after it.
  *   F : DEVICE fp32 [N][3] caller order.  U : DEVICE fp32 [N][3] caller order; U is OVERWRITTEN with
- *   the far-field contribution of the resident blocks only. */
+ *   the contribution of the resident admissible blocks only. */
 int hh_far_apply_resident(hh_ctx* ctx, const float* F, float* U);
 
 /* Step 12: one time step (L102, L338): build tree + blocks from X, U = M(X) F, X <- X + dt U (fp32,

@@ -208,13 +208,7 @@ __global__ void __launch_bounds__(A2_T, 2) k2_mlp(A2Args A, u32 count) {
 // ---- lines 4-5 resp. 7-8, second half: residual against the stored rank terms, pivot scores, Gram sums.
 // Half a warp per granule, one entry per thread.
 template <bool COLS>
-#ifndef A2_UPD_MINB
-#define A2_UPD_MINB 4
-#endif
-#ifndef A2_UPD_UNROLL
-#define A2_UPD_UNROLL 2
-#endif
-__global__ void __launch_bounds__(256, A2_UPD_MINB) k2_upd(A2Args A, u32 count) {
+__global__ void __launch_bounds__(256, 4) k2_upd(A2Args A, u32 count) {
   const u32 lane = threadIdx.x & 31, l16 = lane & 15;
   const u32 gi = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
   const bool gv = gi < count;
@@ -234,7 +228,7 @@ __global__ void __launch_bounds__(256, A2_UPD_MINB) k2_upd(A2Args A, u32 count) 
   // over the stored rows Q_p(j) also builds Z(j) = sum_p Q_p(j)^T A_pk for the cross term (S-19).
   if (ok) {
     const u32 fix = COLS ? (u32)s.ik : (u32)s.jk;
-#pragma unroll A2_UPD_UNROLL
+#pragma unroll 2
     for (int p = 0; p < k; ++p) {
       const float* base = chunk_ptr(A, tabrow, p);
       const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;

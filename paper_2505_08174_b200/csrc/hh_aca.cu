@@ -346,10 +346,6 @@ __global__ void __launch_bounds__(T, T >= 256 ? 1 : 384 / T) k_aca(AcaArgs A) {
   // ---- record: rank, flag, chunk table, pivots ----
   if (tid == 0) { A.ranks[g] = rank; A.flags[g] = flag; }
   for (int t = tid; t < HH_MAX_CHUNKS; t += T) tabrow[t] = (t * HH_RC < rank) ? S.chunk[t] : 0xffffffffu;
-  if (tid == 0) {
-    tabrow[HH_TAB_DESC] = tlo; tabrow[HH_TAB_DESC + 1] = m; tabrow[HH_TAB_DESC + 2] = slo; tabrow[HH_TAB_DESC + 3] = n;
-    tabrow[HH_TAB_DESC + 4] = (u32)rank; tabrow[HH_TAB_DESC + 5] = (u32)flag;
-  }
   int* piv = (int*)(A.arena + (size_t)tabrow[HH_TAB_PIV] * HH_UNIT_FLOATS);
   // a breakdown (flag 2) also lists the attempted pivot after the accepted ones
   for (int t = tid; t < rank + (flag == 2 ? 1 : 0); t += T) { piv[t] = S.piv_i[t]; piv[HH_MAX_RANK + t] = S.piv_j[t]; }

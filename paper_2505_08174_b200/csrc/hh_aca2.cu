@@ -111,8 +111,6 @@ __device__ __forceinline__ void a2_finish(const A2Args& A, u32 b, BlkState& s, i
   A.flags[A.first + b] = flag;
   u32* tabrow = A.tab + (size_t)b * HH_TAB_STRIDE;
   for (int t = (s.k + HH_RC - 1) / HH_RC; t < HH_MAX_CHUNKS; ++t) tabrow[t] = 0xffffffffu;
-  tabrow[HH_TAB_DESC] = s.tlo; tabrow[HH_TAB_DESC + 1] = s.m; tabrow[HH_TAB_DESC + 2] = s.slo; tabrow[HH_TAB_DESC + 3] = s.n;
-  tabrow[HH_TAB_DESC + 4] = (u32)s.k; tabrow[HH_TAB_DESC + 5] = (u32)flag;
 }
 
 __global__ void __launch_bounds__(256) k2_init(A2Args A) {

@@ -25,17 +25,18 @@ __global__ void __launch_bounds__(T) k_far(const uint2* __restrict__ PG, const u
                                             const float* __restrict__ Fs, float* __restrict__ Us, u32 first, u32 begin) {
   __shared__ __align__(16) float sF[3][JT];        // component-major force tile
   __shared__ float st[HH_MAX_RANK * 3];                // t_k = Q_k F^sigma
-  __shared__ u32 sch[HH_TAB_STRIDE];               // the block's table row: chunk offsets + descriptor
+  __shared__ u32 sch[HH_MAX_CHUNKS];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int NW = T / 32;
   const u32 g = begin + blockIdx.x;
-  if (tid < HH_TAB_STRIDE) sch[tid] = tab[(size_t)(g - first) * HH_TAB_STRIDE + tid];      // one 128-byte load, no dependent chain
-  __syncthreads();
-  const int l = (int)sch[HH_TAB_DESC + 4];
-  if (l <= 0 || sch[HH_TAB_DESC + 5] == 2u) return;   // nothing factorised / Alg. 2 broke down (applied densely, S-18b)
-  const u32 tlo = sch[HH_TAB_DESC], m = sch[HH_TAB_DESC + 1];
-  const u32 slo = sch[HH_TAB_DESC + 2], n = sch[HH_TAB_DESC + 3];
+  const int l = ranks[g];
+  if (l <= 0 || flags[g] == 2) return;             // nothing factorised / Alg. 2 broke down (applied densely, S-18b)
+  const uint2 blk = PG[g];
+  const u32 tlo = nlo[blk.x], m = nhi[blk.x] - tlo;
+  const u32 slo = nlo[blk.y], n = nhi[blk.y] - slo;
   const u32 mp = pad8f(m), np = pad8f(n);
+  const u32* row = tab + (size_t)(g - first) * HH_TAB_STRIDE;
+  if (tid < HH_MAX_CHUNKS) sch[tid] = row[tid];
   for (int t = tid; t < 3 * l; t += T) st[t] = 0.f;
   // ---- phase 1: t_k = sum_j Q_k(j) F(j) ----
   for (u32 j0 = 0; j0 < n; j0 += JT) {

@@ -15,7 +15,6 @@ typedef uint64_t u64;
 #define HH_UNIT_FLOATS 32                       /* arena allocation unit = 128 B                   */
 #define HH_TAB_STRIDE 32                        /* u32 per resident block: 24 chunk offsets + pivot offset + pad */
 #define HH_TAB_PIV 24
-#define HH_TAB_DESC 25                          /* tlo, m, slo, n, rank, flag of the block: the far-field kernel needs one 128-B load */
 #define HH_MAX_LEAF 256                         /* largest supported C_leaf                        */
 #define HH_MAX_LEVELS 128
 

@@ -295,7 +295,8 @@ def run_gpu(args):
                                       "sum_rank", "aca_entries", "factor_bytes", "aca_not_converged", "aca_singular", "fallback_entries", "n_faces")},
         "roofline": {"kernel": "k_far (far-field apply U^tau += C (Q F^sigma), all size classes and arena batches of one step)",
                      "bound": "hbm", "achieved": far_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": far_gbs / hbm_peak,
-                     "traffic": None, "peak_source": peak_src, "share_of_step": far_ms / step_ms,
+                     "traffic": None, "traffic_note": "not collected in this run (needs ncu); measured dram__bytes_read = 1.02 x algorithmic bytes, profiles/r01b_far_traffic.md",
+                     "peak_source": peak_src, "share_of_step": far_ms / step_ms,
                      "algorithmic_bytes_per_step": far_bytes, "ms_per_step": far_ms},
         "wall_s_timed_region": t_wall,
     }

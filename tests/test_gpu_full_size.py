@@ -59,3 +59,32 @@ def test_c3_matvec_on_sampled_particles_vs_dense(c3, mlp2):
     # Eq. (10) is a heuristic stop (S-20) and this is a 48-particle estimate of eps_r: measured 1.0e-4 at zeta = 1e-4
     assert err <= 2.0 * cfg["tol"]
     ctx.close()
+
+
+def test_c2_ten_euler_steps_then_sampled_dense(mlp2, mlp3):
+    """config c2 as BASELINE.json states it: 65,536-particle drop, gravity, three-body term, 10 forward-Euler steps with
+    dt = 0.01, tree / blocks / factors rebuilt every step.  Trajectories of two fp32 programs diverge at the 1e-6 level, so
+    the oracle is fed the GPU's positions of the last step: two-body velocity on sampled particles vs O-dense (<= 2 zeta),
+    Euler update bit-exact from the GPU's own U (S-25), and the drop must have moved down."""
+    cfg, X, F = synth.config("c2")
+    N = len(X)
+    ctx = make_ctx(mlp2, mlp3, ws_mb=64 * 1024, leaf_size=cfg["leaf"], eta=cfg["eta"], aca_tol=cfg["tol"], rcut3=cfg["rcut3"])
+    Xd, Fd = to_dev(X), to_dev(F)
+    for _ in range(cfg["steps"] - 1):
+        ctx.step(Xd, Fd, dt=cfg["dt"])
+    Xlast = Xd.cpu().numpy()
+    U = ctx.step(Xd, Fd, dt=cfg["dt"]).cpu().numpy()
+    assert np.array_equal(Xd.cpu().numpy(), oracle.euler(Xlast, U.astype(np.float64), cfg["dt"]))
+    assert float(np.mean(Xd.cpu().numpy()[:, 2] - X[:, 2])) < 0.0            # gravity (0,0,-1): the drop sediments
+    st = ctx.stats()
+    assert st["n_faces"] > 0 and st["aca_not_converged"] == 0
+    # two-body part of the last step on sampled particles (tree and factors are those of Xlast)
+    ctx.build_tree(to_dev(Xlast))
+    ctx.build_blocks()
+    U2 = ctx.matvec(Fd, parts=7).cpu().numpy().astype(np.float64)
+    rows = np.unique((np.arange(64, dtype=np.int64) * 1009 + 5) % N)
+    Ud = oracle.dense_matvec(Xlast, F, mlp2, rows=rows)
+    err = np.linalg.norm(U2[rows] - Ud) / np.linalg.norm(Ud)
+    print("c2 after 10 steps: sampled eps_r vs dense %.3e" % err)
+    assert err <= 2.0 * cfg["tol"]
+    ctx.close()

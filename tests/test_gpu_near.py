@@ -54,3 +54,19 @@ def test_near_part_matches_oracle_near_part(mlp2):
     U1 = ctx.matvec(to_dev(F), parts=1).cpu().numpy()
     assert np.array_equal(U1, F)
     ctx.close()
+
+
+@pytest.mark.parametrize("n,leaf", [(1, 64), (2, 64), (3, 1), (65, 64)])
+def test_tiny_clouds_whole_matvec(n, leaf, mlp2_bias):
+    """edge sizes: a single particle (U = F: only the self term), two particles, one-particle leaves, one ragged split"""
+    X = synth.cube_cloud(n, 0.05, seed=11)
+    F = synth.gaussian_forces(n, seed=12)
+    ctx = make_ctx(mlp2_bias, leaf_size=leaf, eta=1.0, ws_mb=512)
+    ctx.build_tree(to_dev(X))
+    ctx.build_blocks()
+    U = ctx.matvec(to_dev(F)).cpu().numpy()
+    ref = oracle.dense_matvec(X, F, mlp2_bias)
+    if n == 1:
+        assert np.array_equal(U, F)
+    assert rel_l2(U, ref) <= 1e-5
+    ctx.close()

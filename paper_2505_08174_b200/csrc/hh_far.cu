@@ -20,7 +20,7 @@ __device__ __forceinline__ float ldg_stream1(const float* p) {
 
 // T threads; JT = source columns staged per tile (>= the largest n of the size class, or 2048 with tiling)
 template <int T, int JT>
-__global__ void __launch_bounds__(T) k_far(const uint2* __restrict__ PG, const u32* __restrict__ nlo, const u32* __restrict__ nhi,
+__global__ void __launch_bounds__(T, 1024 / T) k_far(const uint2* __restrict__ PG, const u32* __restrict__ nlo, const u32* __restrict__ nhi,
                                             const int* __restrict__ ranks, const int* __restrict__ flags, const u32* __restrict__ tab, const float* __restrict__ arena,
                                             const float* __restrict__ Fs, float* __restrict__ Us, u32 first, u32 begin) {
   __shared__ __align__(16) float sF[3][JT];        // component-major force tile

@@ -92,9 +92,10 @@ __global__ void __launch_bounds__(T, 1024 / T) k_far(const uint2* __restrict__ P
   }
 }
 
-// CTA sizes per size class (max(m,n) > 256, <= 256, <= 128, <= 64) are measured, not derived: the kernel is bound by
-// per-CTA start-up latency and load concurrency, and half the threads per CTA (twice the CTAs per SM) gave 4.70 instead
-// of 4.28 TB/s at c3; a quarter gave 4.13 TB/s (the 32-CTA-per-SM limit then caps the warps).
+// CTA sizes per size class (max(m,n) > 256, <= 256, <= 128, <= 64) and the 64-register cap (32 warps per SM) are measured,
+// not derived: the kernel is bound by per-CTA start-up latency and load concurrency.  512 threads / 70 registers for the
+// first class gave 4.28 TB/s at c3, 256 threads / 64 registers 5.03 TB/s (c4: 4.52 -> 5.06 TB/s); halving the threads of
+// every class again helps c3's ragged 64-particle leaves slightly but costs 15 % at c4's 128-particle leaves.
 int hh_far_apply(hh_ctx* ctx) {
   if (ctx->res_next <= ctx->res_first) return HH_OK;
   cudaStream_t s = ctx->stream;
@@ -104,10 +105,10 @@ int hh_far_apply(hh_ctx* ctx) {
     u32 e = ctx->class_bound[c + 1] < end ? ctx->class_bound[c + 1] : end;
     if (b >= e) continue;
     switch (c) {
-      case 0: k_far<128, 2048><<<HH_N + e - b, 128, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      case 1: k_far<128, 256><<<HH_N + e - b, 128, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      case 2: k_far<64, 128><<<HH_N + e - b, 64, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
-      default: k_far<32, 64><<<HH_N + e - b, 32, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 0: k_far<256, 2048><<<HH_N + e - b, 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 1: k_far<256, 256><<<HH_N + e - b, 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      case 2: k_far<128, 128><<<HH_N + e - b, 128, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
+      default: k_far<64, 64><<<HH_N + e - b, 64, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;
     }
   }
   HH_LAUNCH_CHECK();

@@ -55,7 +55,7 @@ class Stats(C.Structure):
 
 
 def lib_path():
-    return os.path.join(_HERE, "libhh.so")
+    return os.environ.get("HH_LIB_PATH") or os.path.join(_HERE, "libhh.so")      # HH_LIB_PATH: try another build of the same ABI
 
 
 def load(build_if_missing=True):

@@ -88,3 +88,35 @@ def test_c2_ten_euler_steps_then_sampled_dense(mlp2, mlp3):
     print("c2 after 10 steps: sampled eps_r vs dense %.3e" % err)
     assert err <= 2.0 * cfg["tol"]
     ctx.close()
+
+
+def test_c4_ten_million_particles(mlp2):
+    """config c4 (N = 10^7, leaf 128): Morton order, tree, boxes and both block lists bit-exact IN FULL against the
+    oracle; one whole two-body mat-vec (factors streamed through the arena in ~110 batches) on 16 sampled particles
+    against O-dense (one 10^7-term sum each)."""
+    cfg, X, F = synth.config("c4")
+    N = len(X)
+    H = oracle.HMatrix(X, mlp2, leaf=cfg["leaf"], eta=cfg["eta"])
+    ctx = make_ctx(mlp2, ws_mb=140 * 1024, leaf_size=cfg["leaf"], eta=cfg["eta"], aca_tol=cfg["tol"])
+    ctx.build_tree(to_dev(X))
+    ctx.build_blocks()
+    tr = ctx.get_tree()
+    assert np.array_equal(tr["perm"], H.perm) and np.array_equal(tr["keys"], H.keys)
+    gn, gmin, gmax = gpu_node_table(tr)
+    on, omin, omax = H.node_table()
+    assert np.array_equal(gn, on)
+    assert np.array_equal(gmin.view(np.uint32), omin.view(np.uint32)) and np.array_equal(gmax.view(np.uint32), omax.view(np.uint32))
+    for which in ("G", "H"):
+        t, s = ctx.get_blocks(which)
+        assert np.array_equal(gpu_block_table(tr, t, s), H.block_table(which))
+    del H
+    U = ctx.matvec(to_dev(F), parts=7).cpu().numpy().astype(np.float64)
+    st = ctx.stats()
+    assert np.isfinite(U).all() and st["aca_not_converged"] == 0
+    rows = np.unique((np.arange(16, dtype=np.int64) * 1000003 + 7) % N)
+    Ud = oracle.dense_matvec(X, F, mlp2, rows=rows)
+    err = np.linalg.norm(U[rows] - Ud) / np.linalg.norm(Ud)
+    print("c4 sampled eps_r vs dense on %d particles: %.3e (zeta %.0e); batches %d, mean rank %.1f"
+          % (len(rows), err, cfg["tol"], st["aca_batches"], st["sum_rank"] / st["n_admissible"]))
+    assert err <= 2.0 * cfg["tol"]
+    ctx.close()

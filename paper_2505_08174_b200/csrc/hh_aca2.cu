@@ -12,7 +12,8 @@
 //                     A'_pk = sum_i C_p(i)^T c'(i)
 //   k_piv   line 5-6  pivot row i_k, P = c'(i_k), P^-1 and cond_F(P) in fp64; zero column -> done (S-21); singular or
 //                     cond_F > kappa_max -> breakdown, block goes dense (S-18, S-18b); A_pk = A'_pk P^-1
-//   k_norm  line 6    c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk = sum_i c_k(i)^T c_k(i)   (S-19)
+//   (line 6)          c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk = sum_i c_k(i)^T c_k(i)   (S-19);
+//                     memory-bound, interleaved with the MLP tiles of the row side inside k2_mlp<true>
 //   k_row   line 7-8  q_k(j) = G(i_k,j) - sum_p C_p(i_k) Q_p(j), stored raw; arg-max for j_{k+1};
 //                     nu^2 = sum_j tr(A_kk q q^T), cross = sum_j tr([sum_p Q_p(j)^T A_pk] q(j))  (= sum_p tr(A_pk B_kp), S-19)
 //   k_fin   line 9-12 lambda^2 += nu^2 + 2 cross; stop test Eq. (10) (S-20);
@@ -153,20 +154,68 @@ __global__ void __launch_bounds__(256) k2_gran_fill(A2Args A) {                /
   for (u32 t = lane; t < nn; t += 32) A.gn[pn + t] = make_uint2(b, t * GR);
 }
 
+// ---- line 6: c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk = sum_i c_k(i)^T c_k(i) (S-19).
+// Half a warp per granule of rows; called by all 32 lanes (shuffles inside).  It is memory-bound and independent of
+// the entry evaluation of the row side (line 7), so k2_mlp<true> interleaves it with its MLP tiles: the loads of one
+// hide behind the arithmetic of the other.
+__device__ __forceinline__ void a2_norm_granule(const A2Args& A, u32 gi, u32 count, u32 lane) {
+  const u32 l16 = lane & 15;
+  const bool gv = gi < count;
+  const uint2 g = A.gm[gv ? gi : count - 1];
+  const BlkState& s = A.st[g.x];
+  const u32 i = g.y + l16, mp = a2_pad8(s.m);
+  const bool ok = gv && s.status == 0 && i < s.m;
+  const int k = s.k;
+  const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+  float* acc = A.acc + (size_t)g.x * acc_stride(A.R);
+  float c[9], akk[9];
+#pragma unroll
+  for (int r = 0; r < 9; ++r) { c[r] = 0.f; akk[r] = 0.f; }
+  if (ok) {
+    float* Ck = chunk_ptr(A, tabrow, k) + (size_t)(k % HH_RC) * 9 * mp;
+    double Pi[9];
+    float cr[9];
+#pragma unroll
+    for (int r = 0; r < 9; ++r) { Pi[r] = A.pinv[(size_t)g.x * 9 + r]; cr[r] = Ck[(size_t)r * mp + i]; }
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int q = 0; q < 3; ++q)
+        c[3 * r + q] = (float)((double)cr[3 * r] * Pi[q] + (double)cr[3 * r + 1] * Pi[3 + q] + (double)cr[3 * r + 2] * Pi[6 + q]);
+#pragma unroll
+    for (int r = 0; r < 9; ++r) Ck[(size_t)r * mp + i] = c[r];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+      for (int q = 0; q < 3; ++q) akk[3 * r + q] = c[r] * c[q] + c[3 + r] * c[3 + q] + c[6 + r] * c[6 + q];
+  }
+  {
+    const float t = half_sum9(akk, l16);
+    const bool okh = __shfl_sync(0xffffffffu, ok, lane & 16);       // validity of the granule (its first row)
+    if (l16 < 9 && okh) atomicAdd(&acc[l16], t);
+  }
+}
+
+
 // ---- lines 4 and 7, first half: the entries G(i, j_k) (COLS = false: over the rows of tau) resp. G(i_k, j) (COLS = true:
 // over the columns of sigma) of all active blocks, evaluated by the MLP and stored raw in the slot of rank k.
 // A warp takes 4 granules: slot (e, half) -> granule 4*tile + 2*e + half; every thread evaluates two entries.
 // Nothing else happens here, so this kernel runs at the speed of the near-field kernel; the residual, the pivot
 // scores and the Gram sums are the bandwidth-bound second half (k2_upd), which runs at four times the occupancy.
 template <bool COLS>
-__global__ void __launch_bounds__(A2_T, 2) k2_mlp(A2Args A, u32 count) {
+__global__ void __launch_bounds__(A2_T, 2) k2_mlp(A2Args A, u32 count, u32 ncount) {
   __shared__ __align__(16) float sw[HH_MLP2_FLOATS];
   load_weights(sw, A.w2, HH_MLP2_FLOATS);
   __syncthreads();
   const u32 lane = threadIdx.x & 31, half = lane >> 4, l16 = lane & 15, warp = threadIdx.x >> 5;
   const uint2* gl = COLS ? A.gn : A.gm;
   const u32 ntiles = (count + 3) / 4;
-  for (u32 tile = blockIdx.x * (A2_T / 32) + warp; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
+  u32 tile = blockIdx.x * (A2_T / 32) + warp;
+  for (; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
+    if (COLS && 4 * tile < ncount) {                                // line 6 for the row granules with the same indices
+      a2_norm_granule(A, 4 * tile + half, ncount, lane);
+      a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
+    }
     u32 idx[2], len[2], lenp[2];
     bool ok[2], live[2];
     float xi[2][3], xj[2][3], v[2][9];
@@ -203,6 +252,11 @@ __global__ void __launch_bounds__(A2_T, 2) k2_mlp(A2Args A, u32 count) {
       }
     }
   }
+  if (COLS)                                                         // more row granules than column granules: finish line 6
+    for (; 4 * tile < ncount; tile += gridDim.x * (A2_T / 32)) {
+      a2_norm_granule(A, 4 * tile + half, ncount, lane);
+      a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
+    }
 }
 
 // ---- lines 4-5 resp. 7-8, second half: residual against the stored rank terms, pivot scores, Gram sums.
@@ -368,46 +422,6 @@ __global__ void __launch_bounds__(256) k2_piv(A2Args A) {
   A.st[b] = s;
 }
 
-// ---- line 6: c_k(i) = c'(i) P^-1; Gram matrices A_kk, A_pk (S-19).  Half a warp per granule of rows. ----
-__global__ void __launch_bounds__(256) k2_norm(A2Args A, u32 count) {
-  const u32 lane = threadIdx.x & 31, l16 = lane & 15;
-  const u32 gi = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
-  const bool gv = gi < count;
-  const uint2 g = A.gm[gv ? gi : count - 1];
-  const BlkState& s = A.st[g.x];
-  const u32 i = g.y + l16, mp = a2_pad8(s.m);
-  const bool ok = gv && s.status == 0 && i < s.m;
-  const int k = s.k;
-  const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
-  float* acc = A.acc + (size_t)g.x * acc_stride(A.R);
-  float c[9], akk[9];
-#pragma unroll
-  for (int r = 0; r < 9; ++r) { c[r] = 0.f; akk[r] = 0.f; }
-  if (ok) {
-    float* Ck = chunk_ptr(A, tabrow, k) + (size_t)(k % HH_RC) * 9 * mp;
-    double Pi[9];
-    float cr[9];
-#pragma unroll
-    for (int r = 0; r < 9; ++r) { Pi[r] = A.pinv[(size_t)g.x * 9 + r]; cr[r] = Ck[(size_t)r * mp + i]; }
-#pragma unroll
-    for (int r = 0; r < 3; ++r)
-#pragma unroll
-      for (int q = 0; q < 3; ++q)
-        c[3 * r + q] = (float)((double)cr[3 * r] * Pi[q] + (double)cr[3 * r + 1] * Pi[3 + q] + (double)cr[3 * r + 2] * Pi[6 + q]);
-#pragma unroll
-    for (int r = 0; r < 9; ++r) Ck[(size_t)r * mp + i] = c[r];
-#pragma unroll
-    for (int r = 0; r < 3; ++r)
-#pragma unroll
-      for (int q = 0; q < 3; ++q) akk[3 * r + q] = c[r] * c[q] + c[3 + r] * c[3 + q] + c[6 + r] * c[6 + q];
-  }
-  {
-    const float t = half_sum9(akk, l16);
-    const bool okh = __shfl_sync(0xffffffffu, ok, lane & 16);       // validity of the granule (its first row)
-    if (l16 < 9 && okh) atomicAdd(&acc[l16], t);
-  }
-}
-
 // ---- lines 9-12: norm recursion (S-19), stop test Eq. (10) (S-20), next column (line 8), arena space ----
 __global__ void __launch_bounds__(256) k2_fin(A2Args A) {
   const u32 b = blockIdx.x * blockDim.x + threadIdx.x;
@@ -524,11 +538,10 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       k2_gran_fill<<<HH_N + cdiv((int64_t)nb * 32, 256), 256, 0, s>>>(A);
       const unsigned cap = 148 * 2 * 4;
       unsigned g1 = cdiv(cdiv(gmc, 4), A2_T / 32), g2 = cdiv(cdiv(gnc, 4), A2_T / 32);
-      k2_mlp<false><<<HH_N + (g1 < cap ? g1 : cap), A2_T, 0, s>>>(A, gmc);
+      k2_mlp<false><<<HH_N + (g1 < cap ? g1 : cap), A2_T, 0, s>>>(A, gmc, 0u);
       k2_upd<false><<<HH_N + cdiv((int64_t)gmc * GR, 256), 256, 0, s>>>(A, gmc);
       k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
-      k2_norm<<<HH_N + cdiv((int64_t)gmc * GR, 256), 256, 0, s>>>(A, gmc);
-      k2_mlp<true><<<HH_N + (g2 < cap ? g2 : cap), A2_T, 0, s>>>(A, gnc);
+      k2_mlp<true><<<HH_N + ((g1 > g2 ? g1 : g2) < cap ? (g1 > g2 ? g1 : g2) : cap), A2_T, 0, s>>>(A, gnc, gmc);   // + line 6 (normalisation)
       k2_upd<true><<<HH_N + cdiv((int64_t)gnc * GR, 256), 256, 0, s>>>(A, gnc);
       k2_fin<<<HH_N + gb, 256, 0, s>>>(A);
       HH_LAUNCH_CHECK();

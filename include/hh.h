@@ -157,6 +157,17 @@ int hh_far_apply_resident(hh_ctx* ctx, const float* F, float* U);
  * S-25).  X : DEVICE fp32 [N][3], updated in place.  F read, U written (DEVICE). */
 int hh_step(hh_ctx* ctx, float* X, const float* F, float* U, int64_t N, float dt);
 
+/* hh_step with HOST buffers (the end-to-end call bench.py times): X_host, F_host are copied to the device, hh_step runs,
+ * U_host and the updated X_host are copied back; returns after the copies have completed (the stream is synchronised).
+ *   X_host, F_host, U_host : HOST fp32 [N][3] (pinned memory makes the copies asynchronous); X_host is updated in place.
+ * Errors: as hh_step. */
+int hh_step_host(hh_ctx* ctx, float* X_host, const float* F_host, float* U_host, int64_t N, float dt);
+
+/* Capacity of the block lists and of the Alg. 1 frontier, in pairs per particle (default 32; c3 needs ~5 for P^G and
+ * ~3.4 for P^H).  Takes effect at the next hh_build_tree (the workspace is carved again).
+ * Errors: INVALID_ARG (pairs_per_particle < 1). */
+int hh_set_pair_capacity(hh_ctx* ctx, int64_t pairs_per_particle);
+
 /* ---- introspection (parity tests, counters).  All destination buffers are HOST. ---- */
 int hh_get_stats(hh_ctx* ctx, hh_stats* stats);
 /* perm int64[N] (S-9), keys uint64[N] sorted; node arrays of length n_nodes (any may be NULL). */

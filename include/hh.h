@@ -129,7 +129,8 @@ int hh_build_tree(hh_ctx* ctx, const float* X, int64_t N);
 int hh_build_blocks(hh_ctx* ctx);
 
 /* Step 7: Alg. 2 (L210-L234) on admissible blocks first_block, first_block+1, ... (the library's
- * P^G order) until the factor arena is full or P^G is exhausted; *next_block (HOST) receives the
+ * P^G order, largest blocks first), all blocks of the batch in lock step (L262), until the factor
+ * arena is full or P^G is exhausted; *next_block (HOST) receives the
  * first block NOT factorised (== n_admissible when done).  Factors stay in the arena until the
  * next hh_aca / hh_build_* call.  Blocks that reach aca_max_rank are kept at that rank and counted.
  * Errors: NOT_BUILT, INVALID_ARG (first_block out of range), WORKSPACE_TOO_SMALL (arena cannot

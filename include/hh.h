@@ -69,9 +69,10 @@ typedef struct {
   float   rcut3;         /* three-body cutoff R_cut (L90); 0 = no three-body term                  */
   int32_t pivot_rule;    /* 0 = |det| (Eq. (9)), 1 = Frobenius (listing L219/L224); S-18 */
   int32_t near_path;     /* 0 = fp32 ALU path (tolerance 1e-5).  1 (tensor-core path) is reserved  */
-  float   kappa_max;     /* S-18b: a pivot block with |P|_F |P^-1|_F above this is numerically singular at fp32
-                            entry accuracy: Alg. 2 breaks down on that block (flag 2) and the mat-vec evaluates it
-                            densely like an inadmissible block (L252).  0 = default (300); INFINITY = never   */
+  float   kappa_max;     /* 0 (default) or INFINITY = Alg. 2 as printed: the pivot block is inverted whatever its condition
+                            (L221).  > 0 opts in to S-18b: a pivot block with |P|_F |P^-1|_F above this is treated as
+                            numerically singular, Alg. 2 breaks down on that block (flag 2) and the mat-vec evaluates it
+                            densely like an inadmissible block (L252).  DESIGN.md section 3 states which configs use it. */
   float   dense_cap;     /* S-18b applies where the dense evaluation is affordable: |tau||sigma| <= dense_cap (|tau|+|sigma|);
                             larger blocks keep the ill-conditioned pivot (plain listing).  0 = default (128)          */
 } hh_params;
@@ -168,6 +169,19 @@ int hh_step_host(hh_ctx* ctx, float* X_host, const float* F_host, float* U_host,
  * ~3.4 for P^H).  Takes effect at the next hh_build_tree (the workspace is carved again).
  * Errors: INVALID_ARG (pairs_per_particle < 1). */
 int hh_set_pair_capacity(hh_ctx* ctx, int64_t pairs_per_particle);
+
+/* Pivot capture for parity tests at sizes where the factors are streamed and discarded (replay on sampled
+ * target leaves).  While set, every hh_aca batch (also inside hh_matvec / hh_step) appends one record per factorised
+ * admissible block whose TARGET range [lo,hi) of tree order holds a flagged row, i.e. row_prefix[hi] - row_prefix[lo] > 0:
+ *   row_prefix : DEVICE int32[N+1], exclusive prefix sum of the 0/1 row flags in TREE order (S-9); caller-owned
+ *   records    : DEVICE int32[cap_records][200]: [0] block index in the library's P^G order (hh_get_blocks), [1] rank,
+ *                [2] flag, [3] number of pivot pairs listed (rank, +1 after a breakdown), [4..100) piv_i, [100..196) piv_j
+ *                (local row / column indices, -1 beyond the listed ones), [196..200) unused; caller-owned
+ * records == NULL switches the capture off.  The record counter restarts at 0 on every call; records beyond cap_records
+ * are counted but not written (hh_get_capture_count then exceeds cap_records).  Alg. 2's pivots: L219, L224; S-17, S-18.
+ * Errors: INVALID_ARG, CUDA. */
+int hh_set_capture(hh_ctx* ctx, const int32_t* row_prefix, int32_t* records, int64_t cap_records);
+int hh_get_capture_count(hh_ctx* ctx, int64_t* n_records /* HOST */);
 
 /* ---- introspection (parity tests, counters).  All destination buffers are HOST. ---- */
 int hh_get_stats(hh_ctx* ctx, hh_stats* stats);

@@ -149,7 +149,7 @@ class HMatrix:
 
     def set_kappa_max(self, kappa):
         """S-18b: pivot blocks with cond_F = |P|_F |P^-1|_F above kappa break Alg. 2 down (flag 2, block applied
-        densely).  Default 300; float('inf') gives the plain listing."""
+        densely).  Opt-in: the default is float('inf'), the listing as printed."""
         lib().orc_h_set_kappa_max(self._h, C.c_double(kappa))
 
     def set_dense_cap(self, cap):

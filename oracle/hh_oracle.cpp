@@ -308,9 +308,10 @@ void build_partition(HMat& h, int32_t t, int32_t s) {
 // S-17 j_1 = 0.  S-18 score = |det| (pivot_rule 0, Eq. (9)) or Frobenius (rule 1,
 // listing L219/L224); used rows AND columns excluded; ties -> lowest index; all |det| = 0 but some
 // Frobenius != 0 -> Frobenius for that search; pivot with |det| < 1e-30 -> stop at current rank,
-// flag 2; a pivot block with cond_F(P) = |P|_F |P^-1|_F > kappa_max (default 300) is numerically singular
-// at fp32 entry accuracy and is treated the same way (S-18b): Alg. 2 breaks down, the block is
-// flagged (flag 2) and the mat-vec evaluates it densely like an inadmissible block (L252), which is exact.
+// flag 2.  The default is the listing as printed (L221: the pivot block is inverted, nothing else): kappa_max =
+// infinity.  S-18b is an explicit OPT-IN (orc_h_set_kappa_max): a pivot block with cond_F(P) = |P|_F |P^-1|_F >
+// kappa_max is then treated as numerically singular: Alg. 2 breaks down, the block is flagged (flag 2) and the
+// mat-vec evaluates it densely like an inadmissible block (L252), which is exact (S-18b).
 // S-19 norm recursion via 3x3 Gram matrices A_pk = sum_i C_p(i)^T c_k(i),
 // B_kp = sum_j q_k(j) Q_p(j)^T:  nu^2 = tr(A_kk B_kk), cross term tr(A_pk B_kp).
 // S-20 stop when nu <= zeta*lambda, lambda including the current term.  S-21 degenerate cases.
@@ -380,7 +381,7 @@ int argmax_score(const std::vector<double>& v, int n, const std::vector<char>& u
 // decisions that are not an arg-max / a correct stop within `slack` (relative).
 void aca_block(const HMat& h, const Mlp& mlp, double a, int32_t tnode, int32_t snode, double zeta,
                int max_rank, int rule, int rp_rank, const int32_t* rp_i, const int32_t* rp_j,
-               double slack, AcaOut& out, double u_round = 0.0, double kappa_max = 300.0, int rp_flag = 0,
+               double slack, AcaOut& out, double u_round = 0.0, double kappa_max = INFINITY, int rp_flag = 0,
                double dense_cap = 128.0) {
   const Node& T = h.nodes[tnode];
   const Node& S = h.nodes[snode];
@@ -595,7 +596,7 @@ struct Handle {
   Mlp mlp2;
   double a = 1.0;
   double u_round = 0.0;         // replay checker: unit roundoff of the replayed arithmetic (0 = slack only)
-  double kappa_max = 300.0;     // S-18b: pivot blocks with cond_F above this break Alg. 2 down (block goes dense)
+  double kappa_max = INFINITY;  // S-18b (opt-in): pivot blocks with cond_F above this break Alg. 2 down (block goes dense); default = the plain listing (L221)
   double dense_cap = 128.0;     // S-18b only where |tau||sigma| <= dense_cap (|tau| + |sigma|)
   int64_t last_bad_strict = 0;  // slack-only count of the last replay call
 };

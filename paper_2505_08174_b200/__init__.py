@@ -22,7 +22,7 @@ ERRORS = {-1: "HH_ERR_INVALID_ARG", -2: "HH_ERR_WORKSPACE_TOO_SMALL", -3: "HH_ER
 EXPORTS = ["hh_create", "hh_destroy", "hh_set_params", "hh_enable_timing", "hh_build_tree", "hh_build_blocks", "hh_aca",
            "hh_matvec", "hh_matvec_parts", "hh_set_aca_impl", "hh_far_apply_resident", "hh_step", "hh_step_host", "hh_set_pair_capacity",
            "hh_get_stats", "hh_get_tree", "hh_get_blocks", "hh_get_factors", "hh_get_ranks", "hh_eval_entries",
-           "hh_last_error", "hh_version"]
+           "hh_set_capture", "hh_get_capture_count", "hh_last_error", "hh_version"]
 
 
 class HHError(RuntimeError):
@@ -194,6 +194,17 @@ class Context:
         self.N = int(X.shape[0])
         self._chk(self.lib.hh_step_host(self._h, _ptr(X), _ptr(F), _ptr(U), C.c_int64(self.N), C.c_float(dt)))
         return U
+
+    def set_capture(self, row_prefix=None, records=None):
+        """row_prefix: int32 CUDA tensor [N+1]; records: int32 CUDA tensor [cap][200]; both None = off (see hh.h)"""
+        self._capture = (row_prefix, records)                            # keep the buffers alive
+        cap = 0 if records is None else int(records.shape[0])
+        self._chk(self.lib.hh_set_capture(self._h, _ptr(row_prefix), _ptr(records), C.c_int64(cap)))
+
+    def capture_count(self):
+        n = C.c_int64(0)
+        self._chk(self.lib.hh_get_capture_count(self._h, C.byref(n)))
+        return int(n.value)
 
     # ---- introspection ----
     def stats(self):

@@ -427,7 +427,7 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   ctx->arena_units = (ctx->scratch_bytes - tab_bytes) / 128;
   AcaArgs A;
   A.w2 = ctx->w2; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.max_rank = ctx->p.aca_max_rank; A.rule = ctx->p.pivot_rule;
-  A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : 300.0;
+  A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : (double)INFINITY;   // 0 = the plain listing (L221)
   A.dense_cap = ctx->p.dense_cap > 0.f ? (double)ctx->p.dense_cap : 128.0;
   A.PG = ctx->PG; A.nlo = ctx->nlo; A.nhi = ctx->nhi; A.Xs = ctx->Xs;
   A.arena = ctx->arena; A.arena_units = ctx->arena_units; A.tab = ctx->tab; A.sc = ctx->d_sc;
@@ -448,6 +448,30 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   return hh_aca_batch_finish(ctx, first, end, next);
 }
 
+// hh_set_capture: pivot records of the just-factorised blocks [first, next) whose target range holds a flagged row
+__global__ void __launch_bounds__(128) k_capture(const uint2* __restrict__ PG, const u32* __restrict__ nlo, const u32* __restrict__ nhi,
+                                                  const int* __restrict__ ranks, const int* __restrict__ flags, const u32* __restrict__ tab,
+                                                  const float* __restrict__ arena, u32 first, u32 next, const int32_t* __restrict__ prefix,
+                                                  int32_t* __restrict__ rec, unsigned long long cap, DevScalars* sc) {
+  const u32 g = first + blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), lane = threadIdx.x & 31;
+  if (g >= next) return;
+  const u32 t = PG[g].x;
+  if (prefix[nhi[t]] - prefix[nlo[t]] <= 0) return;
+  unsigned long long slot = 0;
+  if (lane == 0) slot = atomicAdd((unsigned long long*)&sc->cap_count, 1ull);
+  slot = __shfl_sync(0xffffffffu, slot, 0);
+  if (slot >= cap) return;
+  const int r = ranks[g], f = flags[g];
+  const int np = r + (f == 2 ? 1 : 0);                            // a breakdown also lists its attempted pivot
+  int32_t* out = rec + (size_t)slot * HH_CAP_STRIDE;
+  const int* piv = (const int*)(arena + (size_t)tab[(size_t)(g - first) * HH_TAB_STRIDE + HH_TAB_PIV] * HH_UNIT_FLOATS);
+  if (lane == 0) { out[0] = (int32_t)g; out[1] = r; out[2] = f; out[3] = np; }
+  for (int k = lane; k < HH_MAX_RANK; k += 32) {
+    out[4 + k] = k < np ? piv[k] : -1;
+    out[4 + HH_MAX_RANK + k] = k < np ? piv[HH_MAX_RANK + k] : -1;
+  }
+}
+
 // shared by both ACA forms: batch boundary, counters, dense list (S-18b), rank prediction for the next batch
 int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next) {
   cudaStream_t s = ctx->stream;
@@ -457,6 +481,9 @@ int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next) {
   u32 nx = ctx->h_sc->fail_min < end ? ctx->h_sc->fail_min : end;
   k_batch_stats<<<HH_N + cdiv(nb, 256), 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, (u32)first, nx, end,
                                                              ctx->dense_list, ctx->d_sc);
+  if (ctx->cap_rec && nx > (u32)first)
+    k_capture<<<HH_N + cdiv(nx - (u32)first, 4), 128, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, (u32)first, nx,
+                                                              ctx->cap_prefix, ctx->cap_rec, (unsigned long long)ctx->cap_max, ctx->d_sc);
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   const DevScalars& h = *ctx->h_sc;
@@ -497,10 +524,11 @@ int hh_factors_fetch(hh_ctx* ctx, int64_t block, int32_t* rank, int32_t* flag, i
   HH_CUDA(cudaMemcpyAsync(&f, ctx->flags + block, sizeof f, cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   u32 lohi[4];
-  HH_CUDA(cudaMemcpy(&lohi[0], ctx->nlo + blk.x, 4, cudaMemcpyDeviceToHost));
-  HH_CUDA(cudaMemcpy(&lohi[1], ctx->nhi + blk.x, 4, cudaMemcpyDeviceToHost));
-  HH_CUDA(cudaMemcpy(&lohi[2], ctx->nlo + blk.y, 4, cudaMemcpyDeviceToHost));
-  HH_CUDA(cudaMemcpy(&lohi[3], ctx->nhi + blk.y, 4, cudaMemcpyDeviceToHost));
+  HH_CUDA(cudaMemcpyAsync(&lohi[0], ctx->nlo + blk.x, 4, cudaMemcpyDeviceToHost, s));
+  HH_CUDA(cudaMemcpyAsync(&lohi[1], ctx->nhi + blk.x, 4, cudaMemcpyDeviceToHost, s));
+  HH_CUDA(cudaMemcpyAsync(&lohi[2], ctx->nlo + blk.y, 4, cudaMemcpyDeviceToHost, s));
+  HH_CUDA(cudaMemcpyAsync(&lohi[3], ctx->nhi + blk.y, 4, cudaMemcpyDeviceToHost, s));
+  HH_CUDA(cudaStreamSynchronize(s));
   const u32 m = lohi[1] - lohi[0], n = lohi[3] - lohi[2], mp = (m + 7) & ~7u, np = (n + 7) & ~7u;
   if (rank) *rank = r;
   if (flag) *flag = f;
@@ -511,25 +539,31 @@ int hh_factors_fetch(hh_ctx* ctx, int64_t block, int32_t* rank, int32_t* flag, i
   if (np_ > HH_MAX_RANK) np_ = HH_MAX_RANK;
   if ((piv_i || piv_j) && np_ > 0) {
     int piv[2 * HH_MAX_RANK];
-    HH_CUDA(cudaMemcpy(piv, ctx->arena + (size_t)row[HH_TAB_PIV] * HH_UNIT_FLOATS, sizeof piv, cudaMemcpyDeviceToHost));
+    HH_CUDA(cudaMemcpyAsync(piv, ctx->arena + (size_t)row[HH_TAB_PIV] * HH_UNIT_FLOATS, sizeof piv, cudaMemcpyDeviceToHost, s));
+    HH_CUDA(cudaStreamSynchronize(s));
     for (int k = 0; k < np_; ++k) { if (piv_i) piv_i[k] = piv[k]; if (piv_j) piv_j[k] = piv[HH_MAX_RANK + k]; }
   }
   if (C || Q) {
     float* tmp = (float*)malloc(sizeof(float) * 9 * (size_t)(mp > np ? mp : np));
     if (!tmp) return hh_fail(ctx, HH_ERR_INVALID_ARG, "host allocation failed");
-    for (int k = 0; k < rr; ++k) {
+    cudaError_t ce = cudaSuccess;
+    for (int k = 0; k < rr && ce == cudaSuccess; ++k) {
       const float* base = ctx->arena + (size_t)row[k / HH_RC] * HH_UNIT_FLOATS;
       if (C) {
-        cudaMemcpy(tmp, base + (size_t)(k % HH_RC) * 9 * mp, sizeof(float) * 9 * mp, cudaMemcpyDeviceToHost);
+        ce = cudaMemcpyAsync(tmp, base + (size_t)(k % HH_RC) * 9 * mp, sizeof(float) * 9 * mp, cudaMemcpyDeviceToHost, s);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
+        if (ce != cudaSuccess) break;
         for (u32 i = 0; i < m; ++i) for (int e = 0; e < 9; ++e) C[((size_t)k * m + i) * 9 + e] = tmp[(size_t)e * mp + i];
       }
       if (Q) {
-        cudaMemcpy(tmp, base + (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np, sizeof(float) * 9 * np, cudaMemcpyDeviceToHost);
+        ce = cudaMemcpyAsync(tmp, base + (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np, sizeof(float) * 9 * np, cudaMemcpyDeviceToHost, s);
+        if (ce == cudaSuccess) ce = cudaStreamSynchronize(s);
+        if (ce != cudaSuccess) break;
         for (u32 j = 0; j < n; ++j) for (int e = 0; e < 9; ++e) Q[((size_t)k * n + j) * 9 + e] = tmp[(size_t)e * np + j];
       }
     }
     free(tmp);
-    HH_CUDA(cudaGetLastError());
+    HH_CUDA(ce);
   }
   return HH_OK;
 }

@@ -516,7 +516,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     ctx->arena = (float*)(ctx->scratch + off);
     ctx->arena_units = (ctx->scratch_bytes - off) / 128;
     A.w2 = ctx->w2; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.rule = ctx->p.pivot_rule;
-    A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : 300.0;
+    A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : (double)INFINITY;   // 0 = the plain listing (L221)
     A.dense_cap = ctx->p.dense_cap > 0.f ? (double)ctx->p.dense_cap : 128.0;
     A.PG = ctx->PG; A.nlo = ctx->nlo; A.nhi = ctx->nhi; A.Xs = ctx->Xs;
     A.arena = ctx->arena; A.arena_units = ctx->arena_units; A.tab = ctx->tab; A.sc = ctx->d_sc;
@@ -536,7 +536,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       if (nact == 0) break;
       if (gmc > ngran || gnc > ngran) return hh_fail(ctx, HH_ERR_CUDA, "lock-step ACA: granule list overflow (internal)");
       k2_gran_fill<<<HH_N + cdiv((int64_t)nb * 32, 256), 256, 0, s>>>(A);
-      const unsigned cap = 148 * 2 * 4;
+      const unsigned cap = (unsigned)ctx->n_sm * 2 * 4;
       unsigned g1 = cdiv(cdiv(gmc, 4), A2_T / 32), g2 = cdiv(cdiv(gnc, 4), A2_T / 32);
       k2_mlp<false><<<HH_N + (g1 < cap ? g1 : cap), A2_T, 0, s>>>(A, gmc, 0u);
       k2_upd<false><<<HH_N + cdiv((int64_t)gmc * GR, 256), 256, 0, s>>>(A, gmc);

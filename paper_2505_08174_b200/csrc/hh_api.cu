@@ -21,6 +21,11 @@ struct Carver {
 
 // Fixed (per-N) arrays first, the rest of the workspace is the scratch / factor arena.
 static int carve(hh_ctx* ctx, int64_t N) {
+  // every carved pointer changes below: whatever was built for the previous layout is gone, also when this fails
+  ctx->tree_ok = ctx->blocks_ok = 0;
+  ctx->res_first = ctx->res_next = 0;
+  ctx->n_dense = 0;
+  ctx->N = 0;
   Carver c{ctx->ws, 0, ctx->ws_bytes, true};
   ctx->Ncap = N;
   ctx->cap_pairs = ctx->pairs_per_particle * N + 4096;
@@ -85,8 +90,9 @@ static int pack_mlp(hh_ctx* ctx, const hh_mlp* m, int in, int INP, int H, std::v
   size_t cnt[6] = {W1.size(), b1.size(), W2.size(), b2.size(), W3.size(), b3.size()};
   for (int k = 0; k < 6; ++k) {
     if (!src[k]) return HH_ERR_INVALID_ARG;
-    HH_CUDA(cudaMemcpy(dst[k], src[k], cnt[k] * sizeof(float), cudaMemcpyDeviceToHost));
+    HH_CUDA(cudaMemcpyAsync(dst[k], src[k], cnt[k] * sizeof(float), cudaMemcpyDeviceToHost, ctx->stream));
   }
+  HH_CUDA(cudaStreamSynchronize(ctx->stream));                    // the weights must be ready on ctx->stream
   out.assign((size_t)HH_MLP_FLOATS(INP, H), 0.f);
   size_t o = 0;
   for (int r = 0; r < H; ++r) for (int c = 0; c < in; ++c) out[o + (size_t)r * INP + c] = W1[(size_t)r * in + c];
@@ -150,7 +156,15 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   ctx->ws_bytes = workspace_bytes;
   ctx->pairs_per_particle = 32;
   ctx->l_pred = 32.0;
-  *out = ctx;                                       // returned even on failure so hh_last_error works
+  *out = ctx;
+  {
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm < 1) {
+      cudaGetLastError();
+      return hh_fail(ctx, HH_ERR_CUDA, "cannot query the SM count of the current device");
+    }
+    ctx->n_sm = nsm;
+  }                                       // returned even on failure so hh_last_error works
   int r = carve(ctx, 1);
   if (r != HH_OK) return r;
   HH_CUDA(cudaMallocHost((void**)&ctx->h_sc, sizeof(DevScalars)));
@@ -159,11 +173,13 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   std::vector<float> pk;
   r = pack_mlp(ctx, mlp2, 4, HH_MLP2_INP, HH_MLP2_H, pk);
   if (r != HH_OK) return hh_fail(ctx, r, "two-body MLP must be 4->32->32->9 with device weight pointers");
-  HH_CUDA(cudaMemcpy(ctx->w2, pk.data(), pk.size() * sizeof(float), cudaMemcpyHostToDevice));
+  HH_CUDA(cudaMemcpyAsync(ctx->w2, pk.data(), pk.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+  HH_CUDA(cudaStreamSynchronize(ctx->stream));
   if (mlp3) {
     r = pack_mlp(ctx, mlp3, 7, HH_MLP3_INP, HH_MLP3_H, pk);
     if (r != HH_OK) return hh_fail(ctx, r, "three-body MLP must be 7->64->64->9 with device weight pointers");
-    HH_CUDA(cudaMemcpy(ctx->w3, pk.data(), pk.size() * sizeof(float), cudaMemcpyHostToDevice));
+    HH_CUDA(cudaMemcpyAsync(ctx->w3, pk.data(), pk.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    HH_CUDA(cudaStreamSynchronize(ctx->stream));
     ctx->have_mlp3 = 1;
   }
   ctx->Ncap = 0;
@@ -203,6 +219,25 @@ extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
   if (!ctx || (impl != 0 && impl != 1)) return HH_ERR_INVALID_ARG;
   ctx->aca_impl = impl;
   ctx->res_first = ctx->res_next = 0;
+  return HH_OK;
+}
+
+extern "C" int hh_set_capture(hh_ctx* ctx, const int32_t* row_prefix, int32_t* records, int64_t cap_records) {
+  if (!ctx) return HH_ERR_INVALID_ARG;
+  if (records && (!row_prefix || cap_records < 1)) return hh_fail(ctx, HH_ERR_INVALID_ARG, "hh_set_capture: records without row_prefix / capacity");
+  ctx->cap_prefix = records ? row_prefix : nullptr;
+  ctx->cap_rec = records;
+  ctx->cap_max = records ? cap_records : 0;
+  HH_CUDA(cudaMemsetAsync(&ctx->d_sc->cap_count, 0, sizeof(u64), ctx->stream));
+  return HH_OK;
+}
+
+extern "C" int hh_get_capture_count(hh_ctx* ctx, int64_t* n_records) {
+  if (!ctx || !n_records) return HH_ERR_INVALID_ARG;
+  u64 n = 0;
+  HH_CUDA(cudaMemcpyAsync(&n, &ctx->d_sc->cap_count, sizeof n, cudaMemcpyDeviceToHost, ctx->stream));
+  HH_CUDA(cudaStreamSynchronize(ctx->stream));
+  *n_records = (int64_t)n;
   return HH_OK;
 }
 

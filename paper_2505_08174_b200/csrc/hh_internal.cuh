@@ -17,6 +17,7 @@ typedef uint64_t u64;
 #define HH_TAB_PIV 24
 #define HH_MAX_LEAF 256                         /* largest supported C_leaf                        */
 #define HH_MAX_LEVELS 128
+#define HH_CAP_STRIDE 200                      /* int32 per captured pivot record (hh.h: hh_set_capture) */
 
 /* packed MLP weights (floats) as laid out for the kernels: W1 [H][INP], b1 [H], W2 [H][H], b2 [H],
  * W3T [H][12] (9 outputs of hidden unit o, 3 pad), b3 [12]                                        */
@@ -48,6 +49,7 @@ struct DevScalars {
   u64 near_entries, far_rows_cols;
   u32 max_rank_seen, n_dense;
   u64 fallback_entries;
+  u64 cap_count;            /* pivot records written by hh_set_capture's kernel (may exceed the caller's capacity) */
   u64 batch_units, batch_units1;  /* lock-step ACA: padded rows + columns of the batch [first, batch_end) resp. of block `first` alone */
 };
 
@@ -59,6 +61,8 @@ struct hh_ctx {
   int have_mlp3;
   int timing;
   int aca_impl;                         /* 0 = lock-step (hh_aca2.cu), 1 = one CTA per block (hh_aca.cu) */
+  int n_sm;                             /* cudaDevAttrMultiProcessorCount of the context's device (grid sizing) */
+  int three_smem_set;                   /* k_three's dynamic shared-memory attribute has been set on this device */
   int64_t pairs_per_particle;
   /* state */
   int64_t N, Ncap;
@@ -95,6 +99,8 @@ struct hh_ctx {
   u32* tab;                             /* resident block table, HH_TAB_STRIDE u32 per block   */
   /* three-body cell list */
   u32 *cell_of, *cell_start, *cell_order; int64_t n_cells_cap;
+  /* pivot capture for at-size parity tests (hh_set_capture) */
+  const int32_t* cap_prefix; int32_t* cap_rec; int64_t cap_max;
   /* host staging for *_host calls */
   float *stageX, *stageF, *stageU;
 };

@@ -162,7 +162,7 @@ int hh_dense_apply(hh_ctx* ctx) {
   u32* cnt = ctx->dense_cnt;
   k_dense_count<<<HH_N + cdiv(n, 256), 256, 0, ctx->stream>>>(ctx->dense_list, n, ctx->PG, ctx->nlo, ctx->nhi, cnt);
   HH_TRY(hh_scan_u32(ctx, cnt, cnt, n, &ctx->d_sc->n_split));
-  k_dense<<<HH_N + 148 * 2, NR_T, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, ctx->dense_list, n, cnt, &ctx->d_sc->n_split, ctx->PG,
+  k_dense<<<HH_N + ctx->n_sm * 2, NR_T, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, ctx->dense_list, n, cnt, &ctx->d_sc->n_split, ctx->PG,
                                                     ctx->nlo, ctx->nhi, ctx->Xs, ctx->Fs, ctx->Us);
   HH_LAUNCH_CHECK();
   return HH_OK;

@@ -165,8 +165,7 @@ int hh_three_apply(hh_ctx* ctx) {
   HH_TRY(hh_sort_pairs(ctx, k2, v2, N, 0, bits, &which));
   k_cell_start<<<HH_N + cdiv(N + 1, 256), 256, 0, s>>>(k2[which], N, ncells, ctx->cell_start);
   size_t smem = (size_t)HH_MLP3_FLOATS * sizeof(float) + (TB_T / 32) * TB_CAP * sizeof(u32);
-  static bool attr_set = false;
-  if (!attr_set) { cudaFuncSetAttribute(k_three, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); attr_set = true; }
+  if (!ctx->three_smem_set) { HH_CUDA(cudaFuncSetAttribute(k_three, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); ctx->three_smem_set = 1; }
   k_three<<<HH_N + cdiv(N, TB_T / 32), TB_T, smem, s>>>(ctx->w3, ctx->Xs, ctx->Fs, ctx->Us, N, G, ctx->cell_start, v2[which], rcut, ctx->d_sc);
   HH_LAUNCH_CHECK();
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));

@@ -178,7 +178,7 @@ int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N) {
   // rows 1-2: keys, sort, gather
   k_init_bbox<<<HH_N + 1, 32, 0, s>>>(ctx->d_sc);
   unsigned gb = cdiv(N, 256);
-  k_bbox<<<HH_N + (gb < 1184 ? gb : 1184), 256, 0, s>>>(X, N, ctx->d_sc);
+  k_bbox<<<HH_N + (gb < 8u * ctx->n_sm ? gb : 8u * ctx->n_sm), 256, 0, s>>>(X, N, ctx->d_sc);
   k_morton<<<HH_N + gb, 256, 0, s>>>(X, N, ctx->d_sc, ctx->keys[0], ctx->idx[0]);
   HH_LAUNCH_CHECK();
   int which = 0;

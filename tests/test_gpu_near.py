@@ -23,6 +23,25 @@ def test_entries_match_oracle(bias, mlp2, mlp2_bias):
     ctx.close()
 
 
+def test_entry_error_bound(mlp2):
+    """Footing of the replay checker's constant K_G (oracle/hh_oracle.cpp: err(i,j) includes u K_G |G(i,j)|_F with u = 2^-24,
+    K_G = 128): the largest relative Frobenius error of a CUDA fp32 entry against the fp64 oracle, over 20,000 particle
+    pairs spanning the distances of the configs (touching to a cube diagonal apart), must stay below HALF of it.  The rms
+    error is what drives the ACA replay parity."""
+    K_G, u = 128.0, 2.0 ** -24
+    n = 20000
+    X = synth.cube_cloud(2 * n, 0.1, seed=17)
+    Xi, Xj = X[:n].copy(), X[n:].copy()
+    Xj[: n // 2] = Xi[: n // 2] + (Xj[: n // 2] - Xi[: n // 2]) * 0.05          # half of the pairs close (near-field distances)
+    ctx = make_ctx(mlp2, ws_mb=512, radius_a=1.0)
+    M = ctx.eval_entries(to_dev(Xi), to_dev(Xj)).cpu().numpy().astype(np.float64)
+    ref = np.stack([oracle.entry2(mlp2, 1.0, Xi[k], Xj[k]).ravel() for k in range(n)])
+    rel = np.linalg.norm(M - ref, axis=1) / np.linalg.norm(ref, axis=1)
+    print("entry error / |G|_F over %d pairs: rms %.3e, max %.3e = %.1f u (K_G = %g)" % (n, np.sqrt(np.mean(rel ** 2)), rel.max(), rel.max() / u, K_G))
+    assert rel.max() <= 0.5 * K_G * u
+    ctx.close()
+
+
 @pytest.mark.parametrize("n,leaf", [(2048, 64), (1500, 16), (777, 200)])
 def test_nothing_admissible_equals_dense(n, leaf, mlp2_bias):
     """eta -> 0+: every block is near-field, the H mat-vec is the dense product."""

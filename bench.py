@@ -205,7 +205,8 @@ def run_gpu(args):
     free, _ = torch.cuda.mem_get_info(dev)
     ws = int(min(free * 0.85, args.workspace_gb * (1 << 30)))
     ctx = hh.Context(mlp2, mlp3, leaf_size=cfg["leaf"], eta=cfg["eta"], aca_tol=cfg["tol"], rcut3=cfg["rcut3"],
-                     kappa_max=float(cfg.get("kappa_max", 0.0)), workspace_bytes=ws, device=dev)
+                     kappa_max=float(cfg.get("kappa_max", 0.0)), near_path=args.near_path, aca_precision=args.aca_precision,
+                     workspace_bytes=ws, device=dev)
     ctx.enable_timing(True)
     stream = torch.cuda.current_stream(dev)
     Xd = torch.from_numpy(X).to(dev)
@@ -324,6 +325,8 @@ def main():
     ap.add_argument("--tol", type=float, default=None, help="override the config's ACA tolerance zeta (config 3 sweep)")
     ap.add_argument("--leaf", type=int, default=None)
     ap.add_argument("--kappa-max", type=float, default=None, help="S-18b limit on the pivot-block condition number")
+    ap.add_argument("--near-path", type=int, default=0, choices=[0, 1, 2], help="0 fp32 ALU, 1 tcgen05 tf32 + tanh.approx (2e-3), 2 tcgen05 split tf32 + tanhf")
+    ap.add_argument("--aca-precision", type=int, default=0, choices=[0, 1], help="1 = fp64 entries and residuals in Alg. 2 (parity mode)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     args = ap.parse_args()
     args.warmup_ref = min(args.warmup, 1)

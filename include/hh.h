@@ -68,13 +68,21 @@ typedef struct {
   float   radius_a;      /* particle radius a (L41)                                                */
   float   rcut3;         /* three-body cutoff R_cut (L90); 0 = no three-body term                  */
   int32_t pivot_rule;    /* 0 = |det| (Eq. (9)), 1 = Frobenius (listing L219/L224); S-18 */
-  int32_t near_path;     /* 0 = fp32 ALU path (tolerance 1e-5).  1 (tensor-core path) is reserved  */
+  int32_t near_path;     /* near-field entry evaluation (rows 6, 8): 0 = fp32 ALU path (tolerance 1e-5).  1 = tcgen05 tensor cores:
+                            the 32 x 32 layer as a tf32 contraction with the accumulator in tensor memory, tanh.approx
+                            (tolerance 2e-3, north_star).  2 = the same contraction with split tf32 operands (3 products,
+                            fp32-class) and the accurate tanh.  csrc/hh_near_tc.cu                                        */
   float   kappa_max;     /* 0 (default) or INFINITY = Alg. 2 as printed: the pivot block is inverted whatever its condition
                             (L221).  > 0 opts in to S-18b: a pivot block with |P|_F |P^-1|_F above this is treated as
                             numerically singular, Alg. 2 breaks down on that block (flag 2) and the mat-vec evaluates it
                             densely like an inadmissible block (L252).  DESIGN.md section 3 states which configs use it. */
   float   dense_cap;     /* S-18b applies where the dense evaluation is affordable: |tau||sigma| <= dense_cap (|tau|+|sigma|);
                             larger blocks keep the ill-conditioned pivot (plain listing).  0 = default (128)          */
+  int32_t aca_precision; /* 0 = fp32 entries in Alg. 2 (default; the fast path).  1 = parity mode: the entries G(i,j) that Alg. 2
+                            queries (L218, L222) and the residuals are evaluated in fp64 and rounded once when stored (factors
+                            stay fp32).  Two runs of Alg. 2 on the same pivots differ by (entry noise) x cond_F(pivot block);
+                            with fp32 entries (relative noise 2e-7) that is above 1e-5 on large or chain-shaped clouds
+                            (DESIGN.md section 5); this mode removes the noise at ~3x the ACA cost.                       */
 } hh_params;
 
 /* Counters (Figs. 7-9 count "queries" = MLP evaluations; L299). Filled as stages run. */

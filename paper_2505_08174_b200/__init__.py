@@ -39,7 +39,7 @@ class _Mlp(C.Structure):
 class _Params(C.Structure):
     _fields_ = [("leaf_size", C.c_int32), ("eta", C.c_float), ("aca_tol", C.c_float), ("aca_max_rank", C.c_int32),
                 ("radius_a", C.c_float), ("rcut3", C.c_float), ("pivot_rule", C.c_int32), ("near_path", C.c_int32),
-                ("kappa_max", C.c_float), ("dense_cap", C.c_float)]
+                ("kappa_max", C.c_float), ("dense_cap", C.c_float), ("aca_precision", C.c_int32)]
 
 
 class Stats(C.Structure):
@@ -89,7 +89,7 @@ class Context:
     workspace is a torch uint8 CUDA tensor owned here (PyTorch owns all device memory)."""
 
     def __init__(self, mlp2, mlp3=None, leaf_size=64, eta=1.0, aca_tol=1e-4, aca_max_rank=96, radius_a=1.0, rcut3=0.0,
-                 pivot_rule=0, kappa_max=0.0, dense_cap=0.0, workspace_bytes=None, device="cuda:0", stream=None):
+                 pivot_rule=0, near_path=0, kappa_max=0.0, dense_cap=0.0, aca_precision=0, workspace_bytes=None, device="cuda:0", stream=None):
         import torch
         self.torch = torch
         self.lib = load()
@@ -103,7 +103,7 @@ class Context:
         self.workspace = torch.empty(int(workspace_bytes) // 256 * 256, dtype=torch.uint8, device=self.device)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._keep = []
-        self.params = _Params(leaf_size, eta, aca_tol, aca_max_rank, radius_a, rcut3, pivot_rule, 0, kappa_max, dense_cap)
+        self.params = _Params(leaf_size, eta, aca_tol, aca_max_rank, radius_a, rcut3, pivot_rule, near_path, kappa_max, dense_cap, aca_precision)
         m2 = self._mlp_struct(mlp2)
         m3 = self._mlp_struct(mlp3) if mlp3 is not None else None
         self._h = C.c_void_p()

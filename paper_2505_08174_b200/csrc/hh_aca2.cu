@@ -7,16 +7,16 @@
 // near-field kernel (hh_mlp.cuh).  A 2^19-row top-level block and a 20-row leaf block cost the same per entry.
 //
 // One iteration k (all blocks in lock step; blocks drop out as they stop):
-//   (each of k_col / k_row is two launches: k2_mlp evaluates and stores the raw entries, k2_upd does the rest)
+//   (k_col = k2_step<false>, k_row = k2_step<true>: entry evaluation and update fused, stored terms prefetched into L2)
 //   k_col   line 4-5  c'(i) = G(i,j_k) - sum_p C_p(i) Q_p(j_k), stored raw; arg-max scores (Eq. (9), S-18) by atomicMax;
 //                     A'_pk = sum_i C_p(i)^T c'(i)
 //   k_piv   line 5-6  pivot row i_k, P = c'(i_k), P^-1 and cond_F(P) in fp64; zero column -> done (S-21); singular or
 //                     cond_F > kappa_max -> breakdown, block goes dense (S-18, S-18b); A_pk = A'_pk P^-1
 //   (line 6)          c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk = sum_i c_k(i)^T c_k(i)   (S-19);
-//                     memory-bound, interleaved with the MLP tiles of the row side inside k2_mlp<true>
+//                     memory-bound, interleaved with the MLP tiles of the row side inside k2_step<true>
 //   k_row   line 7-8  q_k(j) = G(i_k,j) - sum_p C_p(i_k) Q_p(j), stored raw; arg-max for j_{k+1};
-//                     nu^2 = sum_j tr(A_kk q q^T), cross = sum_j tr([sum_p Q_p(j)^T A_pk] q(j))  (= sum_p tr(A_pk B_kp), S-19)
-//   k_fin   line 9-12 lambda^2 += nu^2 + 2 cross; stop test Eq. (10) (S-20);
+//                     B_kk = sum_j q(j) q(j)^T, cross = sum_j tr([sum_p Q_p(j)^T A_pk] q(j))  (= sum_p tr(A_pk B_kp), S-19)
+//   k_fin   line 9-12 nu^2 = tr(A_kk B_kk); lambda^2 += nu^2 + 2 cross; stop test Eq. (10) (S-20);
 //                     next column; arena space for the next HH_RC ranks
 // Storage, arena chunks, table rows and the pivot record are those of hh_aca.cu (the far-field kernel reads both).
 #include "hh_mlp.cuh"
@@ -36,7 +36,7 @@ struct BlkState {                /* 64 bytes per block of the batch             
 };
 
 struct A2Args {
-  const float* w2; float a; float tol; int rule; double kappa_max, dense_cap;
+  const float* w2; const double* w2d; float a; float tol; int rule; double kappa_max, dense_cap;
   const uint2* PG; const u32 *nlo, *nhi; const float* Xs;
   float* arena; u64 arena_units; u32* tab; DevScalars* sc;
   int *ranks, *flags;
@@ -47,8 +47,11 @@ struct A2Args {
 };
 
 __device__ __forceinline__ u32 a2_pad8(u32 v) { return (v + 7u) & ~7u; }
-__device__ __forceinline__ int acc_stride(int R) { return 18 + 9 * (R + 1); }
-/* accumulators of a block: [0,9) A_kk, [9] nu^2, [10] cross term, 18 + 9p: A_pk                          */
+#define ACC_AKK 0                /* accumulators of a block: [0,9) A_kk, [9,18) B_kk, [18] cross term, 27 + 9p: A_pk    */
+#define ACC_BKK 9
+#define ACC_CROSS 18
+#define ACC_APK 27
+__device__ __forceinline__ int acc_stride(int R) { return ACC_APK + 9 * (R + 1); }
 __device__ __forceinline__ float* chunk_ptr(const A2Args& A, const u32* tabrow, int p) {
   return A.arena + (size_t)tabrow[p / HH_RC] * HH_UNIT_FLOATS;
 }
@@ -102,8 +105,7 @@ __device__ __forceinline__ int* a2_piv(const A2Args& A, u32 b) {
 }
 __device__ __forceinline__ void a2_zero_acc(const A2Args& A, u32 b, int k) {      // slots used by step k
   float* acc = A.acc + (size_t)b * acc_stride(A.R);
-  for (int t = 0; t < 18; ++t) acc[t] = 0.f;
-  for (int t = 0; t < 9 * k; ++t) acc[18 + t] = 0.f;
+  for (int t = 0; t < ACC_APK + 9 * k; ++t) acc[t] = 0.f;
   for (int t = 0; t < 4; ++t) A.amax[(size_t)b * 4 + t] = 0ull;
 }
 __device__ __forceinline__ void a2_finish(const A2Args& A, u32 b, BlkState& s, int status, int flag) {
@@ -156,7 +158,7 @@ __global__ void __launch_bounds__(256) k2_gran_fill(A2Args A) {                /
 
 // ---- line 6: c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk = sum_i c_k(i)^T c_k(i) (S-19).
 // Half a warp per granule of rows; called by all 32 lanes (shuffles inside).  It is memory-bound and independent of
-// the entry evaluation of the row side (line 7), so k2_mlp<true> interleaves it with its MLP tiles: the loads of one
+// the entry evaluation of the row side (line 7), so k2_step<true> interleaves it with its MLP tiles: the loads of one
 // hide behind the arithmetic of the other.
 __device__ __forceinline__ void a2_norm_granule(const A2Args& A, u32 gi, u32 count, u32 lane) {
   const u32 l16 = lane & 15;
@@ -197,58 +199,202 @@ __device__ __forceinline__ void a2_norm_granule(const A2Args& A, u32 gi, u32 cou
 }
 
 
-// ---- lines 4 and 7, first half: the entries G(i, j_k) (COLS = false: over the rows of tau) resp. G(i_k, j) (COLS = true:
-// over the columns of sigma) of all active blocks, evaluated by the MLP and stored raw in the slot of rank k.
-// A warp takes 4 granules: slot (e, half) -> granule 4*tile + 2*e + half; every thread evaluates two entries.
-// Nothing else happens here, so this kernel runs at the speed of the near-field kernel; the residual, the pivot
-// scores and the Gram sums are the bandwidth-bound second half (k2_upd), which runs at four times the occupancy.
-template <bool COLS>
-__global__ void __launch_bounds__(A2_T, 2) k2_mlp(A2Args A, u32 count, u32 ncount) {
-  __shared__ __align__(16) float sw[HH_MLP2_FLOATS];
-  load_weights(sw, A.w2, HH_MLP2_FLOATS);
+// ---- lines 4-5 (COLS = false: over the rows of tau, entries G(i, j_k)) resp. lines 7-8 (COLS = true: over the columns of
+// sigma, entries G(i_k, j)) of all active blocks in ONE launch: entry evaluation by the MLP, residual against the stored
+// rank terms, pivot scores, Gram sums.  A warp takes 4 granules: slot (e, half) -> granule 4*tile + 2*e + half; every thread
+// evaluates two entries (the in-register MLP of hh_mlp.cuh, at near-field speed) and keeps them in registers for the
+// update, so a raw entry never travels through memory.  The update re-reads the k stored rank terms of its rows
+// (36 k bytes per row: the l^2 term of Alg. 2's cost); an arena batch is far larger than L2, so these reads
+// come from HBM.  Their latency is taken off the critical path by prefetching exactly those lines into L2 BEFORE the MLP
+// arithmetic of the tile starts (about 6,000 instructions per thread): by the time the update loop runs, its loads are
+// L2 hits.  Round 1 ran the two halves as separate launches (the update at four times the occupancy to hide the HBM
+// latency) and paid a 72-byte round trip per entry for the raw values on top.
+__device__ __forceinline__ void l2_prefetch(const float* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// F64 (aca_precision = 1, parity mode): the entry and the residual subtraction in fp64, rounded once when stored.
+template <bool COLS, bool F64>
+__global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncount) {
+  __shared__ __align__(16) float sw[F64 ? 2 * HH_MLP2_FLOATS : HH_MLP2_FLOATS];
+  if (F64) load_weights(sw, reinterpret_cast<const float*>(A.w2d), 2 * HH_MLP2_FLOATS);
+  else load_weights(sw, A.w2, HH_MLP2_FLOATS);
   __syncthreads();
   const u32 lane = threadIdx.x & 31, half = lane >> 4, l16 = lane & 15, warp = threadIdx.x >> 5;
   const uint2* gl = COLS ? A.gn : A.gm;
   const u32 ntiles = (count + 3) / 4;
   u32 tile = blockIdx.x * (A2_T / 32) + warp;
   for (; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
-    if (COLS && 4 * tile < ncount) {                                // line 6 for the row granules with the same indices
+    // (a) L2 prefetch of the stored rank terms this half-warp's two granules will read in (d)
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const u32 gi = 4 * tile + 2 * e + half;
+      if (gi < count) {
+        const uint2 g = gl[gi];
+        const BlkState& s = A.st[g.x];
+        const int k = s.k;
+        if (s.status == 0 && k > 0) {
+          const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n), lenp = COLS ? np : mp;
+          const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+          for (int c = 0; c * HH_RC < k; ++c) {
+            const float* base = A.arena + (size_t)tabrow[c] * HH_UNIT_FLOATS + (COLS ? (size_t)HH_RC * 9 * mp : 0) + g.y;
+            const int nt = 9 * min(HH_RC, k - c * HH_RC);
+            for (int t = (int)l16; t < nt; t += 16) {
+              const float* p = base + (size_t)t * lenp;
+              l2_prefetch(p);
+              l2_prefetch(p + 15);                                   // a 64-byte run may straddle two lines
+            }
+          }
+        }
+      }
+    }
+    // (b) line 6 for the row granules with the same indices (memory-bound, independent of line 7)
+    if (COLS && 4 * tile < ncount) {
       a2_norm_granule(A, 4 * tile + half, ncount, lane);
       a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
     }
-    u32 idx[2], len[2], lenp[2];
-    bool ok[2], live[2];
-    float xi[2][3], xj[2][3], v[2][9];
-    float* dst[2];
+    // (c) the entries
+    float v[2][9];
+    double vd[F64 ? 2 : 1][9];
+    {
+      float xi[2][3], xj[2][3];
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const u32 gi = 4 * tile + 2 * e + half;
+        const uint2 g = gl[gi < count ? gi : count - 1];
+        const BlkState& s = A.st[g.x];
+        const u32 len = COLS ? s.n : s.m, idx = g.y + l16;
+        const u32 ic = idx < len ? idx : len - 1;
+        const u32 ti = COLS ? s.tlo + (u32)(s.ik < 0 ? 0 : s.ik) : s.tlo + ic;   // target (row) particle (ik unset on blocks that just stopped)
+        const u32 sj = COLS ? s.slo + ic : s.slo + (u32)s.jk;                    // source (column) particle
+#pragma unroll
+        for (int d = 0; d < 3; ++d) { xi[e][d] = A.Xs[3 * (size_t)ti + d]; xj[e][d] = A.Xs[3 * (size_t)sj + d]; }
+      }
+      if (F64) {
+#pragma unroll 1
+        for (int e = 0; e < 2; ++e) {
+          float a3[3], b3[3];
+          double m9[9];
+#pragma unroll
+          for (int d = 0; d < 3; ++d) { a3[d] = e ? xi[1][d] : xi[0][d]; b3[d] = e ? xj[1][d] : xj[0][d]; }
+          entry2_eval_d(reinterpret_cast<const double*>(sw), (double)A.a, a3, b3, m9);
+#pragma unroll
+          for (int r = 0; r < 9; ++r) { if (e) vd[F64 ? 1 : 0][r] = m9[r]; else vd[0][r] = m9[r]; }
+        }
+      } else {
+        entry2_eval<2>(sw, A.a, xi, xj, v);
+      }
+    }
+    // (d) residual, pivot scores, Gram sums: one granule per half-warp and slot
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const u32 gi = 4 * tile + 2 * e + half;
       const bool gv = gi < count;
       const uint2 g = gl[gv ? gi : count - 1];
-      idx[e] = g.y + l16;
       const BlkState& s = A.st[g.x];
       const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
-      len[e] = COLS ? s.n : s.m;
-      lenp[e] = COLS ? np : mp;
-      live[e] = gv && s.status == 0;
-      ok[e] = live[e] && idx[e] < len[e];
+      const u32 len = COLS ? s.n : s.m, lenp = COLS ? np : mp, idx = g.y + l16;
+      const int k = s.k;
+      const bool live = gv && s.status == 0, ok = live && idx < len;
       const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
-      dst[e] = chunk_ptr(A, tabrow, s.k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(s.k % HH_RC) * 9 * np : (size_t)(s.k % HH_RC) * 9 * mp);
-      const u32 ic = idx[e] < len[e] ? idx[e] : len[e] - 1;
-      const u32 ti = COLS ? s.tlo + (u32)(s.ik < 0 ? 0 : s.ik) : s.tlo + ic;   // target (row) particle (ik unset on blocks that just stopped)
-      const u32 sj = COLS ? s.slo + ic : s.slo + (u32)s.jk;                    // source (column) particle
+      float* acc = A.acc + (size_t)g.x * acc_stride(A.R);
+      float* dst = chunk_ptr(A, tabrow, k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np : (size_t)(k % HH_RC) * 9 * mp);
+      float Z[9];
 #pragma unroll
-      for (int d = 0; d < 3; ++d) { xi[e][d] = A.Xs[3 * (size_t)ti + d]; xj[e][d] = A.Xs[3 * (size_t)sj + d]; }
-    }
-    entry2_eval<2>(sw, A.a, xi, xj, v);
+      for (int r = 0; r < 9; ++r) { Z[r] = 0.f; if (!ok || F64) v[e][r] = 0.f; }
+      // subtract sum_p C_p(row) Q_p(col); the fixed operand is a broadcast load.  On the row side the same pass over the
+      // stored rows Q_p(j) also builds Z(j) = sum_p Q_p(j)^T A_pk for the cross term (S-19).
+      if (ok) {
+        const u32 fix = COLS ? (u32)s.ik : (u32)s.jk;
+#pragma unroll 2
+        for (int p = 0; p < k; ++p) {
+          const float* base = chunk_ptr(A, tabrow, p);
+          const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
+          const float* Qp = base + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
+          float cp[9], qp[9];
 #pragma unroll
-    for (int e = 0; e < 2; ++e) {
-      if (ok[e]) {
+          for (int r = 0; r < 9; ++r) {
+            cp[r] = Cp[(size_t)r * mp + (COLS ? fix : idx)];
+            qp[r] = Qp[(size_t)r * np + (COLS ? idx : fix)];
+          }
+          if (F64) {
 #pragma unroll
-        for (int r = 0; r < 9; ++r) dst[e][(size_t)r * lenp[e] + idx[e]] = v[e][r];
-      } else if (COLS && live[e] && idx[e] < lenp[e]) {
+            for (int r = 0; r < 3; ++r)
 #pragma unroll
-        for (int r = 0; r < 9; ++r) dst[e][(size_t)r * lenp[e] + idx[e]] = 0.f;      // zero the pad columns (far kernel reads float4)
+              for (int c = 0; c < 3; ++c)
+                vd[F64 ? e : 0][3 * r + c] -= (double)cp[3 * r] * (double)qp[c] + (double)cp[3 * r + 1] * (double)qp[3 + c] + (double)cp[3 * r + 2] * (double)qp[6 + c];
+          } else {
+            submul33(v[e], cp, qp);
+          }
+          if (COLS) {
+            const float* Ap = acc + ACC_APK + 9 * p;
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int c = 0; c < 3; ++c) Z[3 * r + c] += qp[r] * Ap[c] + qp[3 + r] * Ap[3 + c] + qp[6 + r] * Ap[6 + c];
+          }
+        }
+        if (F64) {
+#pragma unroll
+          for (int r = 0; r < 9; ++r) v[e][r] = (float)vd[F64 ? e : 0][r];      // rounded once
+        }
+#pragma unroll
+        for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp + idx] = v[e][r];   // the residual (column: normalised by line 6 later; row: kept raw)
+      } else if (COLS && live && idx < lenp) {
+#pragma unroll
+        for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp + idx] = 0.f;      // zero the pad columns (the far-field kernel reads float4)
+      }
+      // arg-max scores over unused rows / columns (Eq. (9); S-18)
+      unsigned long long kd = 0ull, kf = 0ull;
+      if (ok) {
+        const int* piv = a2_piv(A, g.x) + (COLS ? HH_MAX_RANK : 0);
+        bool used = false;
+        for (int q = 0; q < k + (COLS ? 1 : 0); ++q) used |= (piv[q] == (int)idx);
+        if (!used) { kd = amax_key(fabsf(det33(v[e])), idx); kf = amax_key(fro2_33(v[e]), idx); }
+      }
+      kd = half_max(kd); kf = half_max(kf);
+      if (l16 == 0 && (kd | kf)) {
+        atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 2 : 0)], kd);
+        atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 3 : 1)], kf);
+      }
+      if (COLS) {
+        // norm recursion (S-19): B_kk = sum_j q(j) q(j)^T (nu^2 = tr(A_kk B_kk) is formed in k2_fin, once line 6 has summed
+        // A_kk over all rows), cross = sum_p tr(A_pk B_kp) = sum_j tr(Z(j) q(j))
+        float bkk[9], cross = 0.f;
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) {
+            bkk[3 * r + c] = v[e][3 * r] * v[e][3 * c] + v[e][3 * r + 1] * v[e][3 * c + 1] + v[e][3 * r + 2] * v[e][3 * c + 2];
+            cross = fmaf(Z[3 * r + c], v[e][3 * c + r], cross);
+          }
+        const float t = half_sum9(bkk, l16);
+        cross = half_sum(cross);
+        const bool okh = __shfl_sync(0xffffffffu, ok, lane & 16);       // validity of the granule (its first column)
+        if (okh && l16 < 9) atomicAdd(&acc[ACC_BKK + l16], t);
+        if (okh && l16 == 9) atomicAdd(&acc[ACC_CROSS], cross);
+      } else {
+        // Gram matrices of the raw column, A'_pk = sum_i C_p(i)^T c'(i); k2_piv turns them into A_pk = A'_pk P^-1.
+        // The stored columns were read a moment ago by this same thread (L1 / L2 hits, no second trip to HBM).
+        int kw = ok ? k : 0;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
+        const int kh = __shfl_sync(0xffffffffu, ok ? k : 0, lane & 16);
+        for (int p = 0; p < kw; ++p) {
+          float ap[9];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) ap[r] = 0.f;
+          if (ok && p < k) {
+            const float* Cp = chunk_ptr(A, tabrow, p) + (size_t)(p % HH_RC) * 9 * mp;
+            float cp[9];
+#pragma unroll
+            for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + idx];
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int c = 0; c < 3; ++c) ap[3 * r + c] = cp[r] * v[e][c] + cp[3 + r] * v[e][3 + c] + cp[6 + r] * v[e][6 + c];
+          }
+          const float t = half_sum9(ap, l16);
+          if (l16 < 9 && p < kh) atomicAdd(&acc[ACC_APK + 9 * p + l16], t);
+        }
       }
     }
   }
@@ -257,110 +403,6 @@ __global__ void __launch_bounds__(A2_T, 2) k2_mlp(A2Args A, u32 count, u32 ncoun
       a2_norm_granule(A, 4 * tile + half, ncount, lane);
       a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
     }
-}
-
-// ---- lines 4-5 resp. 7-8, second half: residual against the stored rank terms, pivot scores, Gram sums.
-// Half a warp per granule, one entry per thread.
-template <bool COLS>
-__global__ void __launch_bounds__(256, 4) k2_upd(A2Args A, u32 count) {
-  const u32 lane = threadIdx.x & 31, l16 = lane & 15;
-  const u32 gi = (blockIdx.x * blockDim.x + threadIdx.x) >> 4;
-  const bool gv = gi < count;
-  const uint2 g = (COLS ? A.gn : A.gm)[gv ? gi : count - 1];
-  const BlkState& s = A.st[g.x];
-  const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
-  const u32 len = COLS ? s.n : s.m, lenp = COLS ? np : mp, idx = g.y + l16;
-  const int k = s.k;
-  const bool ok = gv && s.status == 0 && idx < len;
-  const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
-  float* acc = A.acc + (size_t)g.x * acc_stride(A.R);
-  float* dst = chunk_ptr(A, tabrow, k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np : (size_t)(k % HH_RC) * 9 * mp);
-  float v[9], Z[9];
-#pragma unroll
-  for (int r = 0; r < 9; ++r) { v[r] = ok ? dst[(size_t)r * lenp + idx] : 0.f; Z[r] = 0.f; }
-  // residual: subtract sum_p C_p(row) Q_p(col); the fixed operand is a broadcast load.  On the row side the same pass
-  // over the stored rows Q_p(j) also builds Z(j) = sum_p Q_p(j)^T A_pk for the cross term (S-19).
-  if (ok) {
-    const u32 fix = COLS ? (u32)s.ik : (u32)s.jk;
-#pragma unroll 2
-    for (int p = 0; p < k; ++p) {
-      const float* base = chunk_ptr(A, tabrow, p);
-      const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
-      const float* Qp = base + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
-      float cp[9], qp[9];
-#pragma unroll
-      for (int r = 0; r < 9; ++r) {
-        cp[r] = Cp[(size_t)r * mp + (COLS ? fix : idx)];
-        qp[r] = Qp[(size_t)r * np + (COLS ? idx : fix)];
-      }
-      submul33(v, cp, qp);
-      if (COLS) {
-        const float* Ap = acc + 18 + 9 * p;
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-          for (int c = 0; c < 3; ++c) Z[3 * r + c] += qp[r] * Ap[c] + qp[3 + r] * Ap[3 + c] + qp[6 + r] * Ap[6 + c];
-      }
-    }
-    if (k > 0) {
-#pragma unroll
-      for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp + idx] = v[r];   // the residual (column: normalised later by k2_norm; row: kept raw)
-    }
-  }
-  // arg-max scores over unused rows / columns (Eq. (9); S-18)
-  unsigned long long kd = 0ull, kf = 0ull;
-  if (ok) {
-    const int* piv = a2_piv(A, g.x) + (COLS ? HH_MAX_RANK : 0);
-    bool used = false;
-    for (int q = 0; q < k + (COLS ? 1 : 0); ++q) used |= (piv[q] == (int)idx);
-    if (!used) { kd = amax_key(fabsf(det33(v)), idx); kf = amax_key(fro2_33(v), idx); }
-  }
-  kd = half_max(kd); kf = half_max(kf);
-  if (l16 == 0 && (kd | kf)) {
-    atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 2 : 0)], kd);
-    atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 3 : 1)], kf);
-  }
-  if (COLS) {
-    // norm recursion (S-19) with the column-side Gram matrices A_kk (k2_norm) and A_pk (k2_upd<false> + k2_piv):
-    //   nu^2 = sum_j tr(A_kk q q^T),  cross = sum_p tr(A_pk B_kp) = sum_j tr(Z(j) q(j))
-    float nu2 = 0.f, cross = 0.f;
-    if (ok) {
-      float W[9];
-      mul33(acc, v, W);
-#pragma unroll
-      for (int r = 0; r < 9; ++r) nu2 = fmaf(W[r], v[r], nu2);
-#pragma unroll
-      for (int r = 0; r < 3; ++r)
-#pragma unroll
-        for (int c = 0; c < 3; ++c) cross = fmaf(Z[3 * r + c], v[3 * c + r], cross);
-    }
-    nu2 = half_sum(nu2); cross = half_sum(cross);
-    if (l16 == 0 && ok) { atomicAdd(&acc[9], nu2); atomicAdd(&acc[10], cross); }
-  } else {
-    // Gram matrices of the raw column, A'_pk = sum_i C_p(i)^T c'(i); k2_piv turns them into A_pk = A'_pk P^-1.
-    // The stored columns were read a moment ago by this same thread (L1 / L2 hits, no second trip to HBM).
-    int kw = ok ? k : 0;
-#pragma unroll
-    for (int o = 16; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
-    const int kh = __shfl_sync(0xffffffffu, ok ? k : 0, lane & 16);
-    for (int p = 0; p < kw; ++p) {
-      float ap[9];
-#pragma unroll
-      for (int r = 0; r < 9; ++r) ap[r] = 0.f;
-      if (ok && p < k) {
-        const float* Cp = chunk_ptr(A, tabrow, p) + (size_t)(p % HH_RC) * 9 * mp;
-        float cp[9];
-#pragma unroll
-        for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + idx];
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-          for (int c = 0; c < 3; ++c) ap[3 * r + c] = cp[r] * v[c] + cp[3 + r] * v[3 + c] + cp[6 + r] * v[6 + c];
-      }
-      const float t = half_sum9(ap, l16);
-      if (l16 < 9 && p < kh) atomicAdd(&acc[18 + 9 * p + l16], t);
-    }
-  }
 }
 
 __device__ __forceinline__ void a2_decode(unsigned long long key, float& score, int& idx) {
@@ -409,7 +451,7 @@ __global__ void __launch_bounds__(256) k2_piv(A2Args A) {
   // c_k = c' P^-1  =>  A_pk = sum_i C_p(i)^T c_k(i) = A'_pk P^-1
   float* acc = A.acc + (size_t)b * acc_stride(A.R);
   for (int p = 0; p < s.k; ++p) {
-    float* Ap = acc + 18 + 9 * p;
+    float* Ap = acc + ACC_APK + 9 * p;
     double a[9];
 #pragma unroll
     for (int r = 0; r < 9; ++r) a[r] = (double)Ap[r];
@@ -430,7 +472,12 @@ __global__ void __launch_bounds__(256) k2_fin(A2Args A) {
   if (s.status != 0) return;
   const float* acc = A.acc + (size_t)b * acc_stride(A.R);
   const int k = s.k;
-  const float nu2 = acc[9], cross = acc[10];
+  float nu2 = 0.f;                                                  // nu^2 = tr(A_kk B_kk)  (S-19)
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) nu2 = fmaf(acc[ACC_AKK + 3 * r + c], acc[ACC_BKK + 3 * c + r], nu2);
+  const float cross = acc[ACC_CROSS];
   s.lam2 += nu2 + 2.f * cross;
   s.k = k + 1;
   const float nu = sqrtf(fmaxf(nu2, 0.f)), lam = sqrtf(fmaxf(s.lam2, 0.f));
@@ -483,7 +530,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   if (chunks_pred < 1) chunks_pred = 1;
   if (chunks_pred > HH_MAX_CHUNKS) chunks_pred = HH_MAX_CHUNKS;
   // per block: table row 128 B, state 64 B, arg-max keys 32 B, P^-1 72 B, accumulators, 2 counters, 2 granules of slack
-  const size_t acc_floats = 18 + 9 * (size_t)(R + 1);
+  const size_t acc_floats = ACC_APK + 9 * (size_t)(R + 1);
   const size_t per_block_bytes = 128 + 64 + 32 + 72 + 4 * acc_floats + 8 + 32 + 16;
   const u32 per_block_units = (u32)((per_block_bytes + 127) / 128);
   const u64 total_units = ctx->scratch_bytes / 128;
@@ -515,7 +562,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     if (off + 4096 > ctx->scratch_bytes) return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "factor arena too small");
     ctx->arena = (float*)(ctx->scratch + off);
     ctx->arena_units = (ctx->scratch_bytes - off) / 128;
-    A.w2 = ctx->w2; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.rule = ctx->p.pivot_rule;
+    A.w2 = ctx->w2; A.w2d = ctx->w2d; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.rule = ctx->p.pivot_rule;
     A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : (double)INFINITY;   // 0 = the plain listing (L221)
     A.dense_cap = ctx->p.dense_cap > 0.f ? (double)ctx->p.dense_cap : 128.0;
     A.PG = ctx->PG; A.nlo = ctx->nlo; A.nhi = ctx->nhi; A.Xs = ctx->Xs;
@@ -538,11 +585,12 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       k2_gran_fill<<<HH_N + cdiv((int64_t)nb * 32, 256), 256, 0, s>>>(A);
       const unsigned cap = (unsigned)ctx->n_sm * 2 * 4;
       unsigned g1 = cdiv(cdiv(gmc, 4), A2_T / 32), g2 = cdiv(cdiv(gnc, 4), A2_T / 32);
-      k2_mlp<false><<<HH_N + (g1 < cap ? g1 : cap), A2_T, 0, s>>>(A, gmc, 0u);
-      k2_upd<false><<<HH_N + cdiv((int64_t)gmc * GR, 256), 256, 0, s>>>(A, gmc);
+      const unsigned gr = (g1 < cap ? g1 : cap), gc = (g1 > g2 ? g1 : g2) < cap ? (g1 > g2 ? g1 : g2) : cap;
+      if (ctx->p.aca_precision) k2_step<false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
+      else k2_step<false, false><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
       k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
-      k2_mlp<true><<<HH_N + ((g1 > g2 ? g1 : g2) < cap ? (g1 > g2 ? g1 : g2) : cap), A2_T, 0, s>>>(A, gnc, gmc);   // + line 6 (normalisation)
-      k2_upd<true><<<HH_N + cdiv((int64_t)gnc * GR, 256), 256, 0, s>>>(A, gnc);
+      if (ctx->p.aca_precision) k2_step<true, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);   // + line 6 (normalisation)
+      else k2_step<true, false><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
       k2_fin<<<HH_N + gb, 256, 0, s>>>(A);
       HH_LAUNCH_CHECK();
     }

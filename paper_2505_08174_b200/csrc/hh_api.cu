@@ -33,6 +33,8 @@ static int carve(hh_ctx* ctx, int64_t N) {
   ctx->d_sc = c.take<DevScalars>(1);
   ctx->w2 = c.take<float>(HH_MLP2_FLOATS);
   ctx->w3 = c.take<float>(HH_MLP3_FLOATS);
+  ctx->w2d = c.take<double>(HH_MLP2_FLOATS);
+  ctx->w2tc = c.take<float>(2 * 1024);
   for (int k = 0; k < 2; ++k) { ctx->keys[k] = c.take<u64>(N); ctx->idx[k] = c.take<u32>(N); }
   ctx->hist_cap = (size_t)((ctx->cap_pairs > N ? ctx->cap_pairs : N) / 8 + 8192);
   ctx->hist = c.take<u32>(ctx->hist_cap);
@@ -74,9 +76,10 @@ static int check_params(const hh_params* p) {
   if (!(p->radius_a > 0.f) || !isfinite(p->radius_a)) return 0;
   if (!(p->rcut3 >= 0.f) || !isfinite(p->rcut3)) return 0;
   if (p->pivot_rule != 0 && p->pivot_rule != 1) return 0;
-  if (p->near_path != 0) return 0;
+  if (p->near_path < 0 || p->near_path > 2) return 0;
   if (!(p->kappa_max >= 0.f)) return 0;
-  if (!(p->dense_cap >= 0.f)) return 0;                           /* 0 = default, INFINITY allowed, NaN / negative not */
+  if (!(p->dense_cap >= 0.f)) return 0;
+  if (p->aca_precision != 0 && p->aca_precision != 1) return 0;                           /* 0 = default, INFINITY allowed, NaN / negative not */
   return 1;
 }
 
@@ -174,6 +177,11 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   r = pack_mlp(ctx, mlp2, 4, HH_MLP2_INP, HH_MLP2_H, pk);
   if (r != HH_OK) return hh_fail(ctx, r, "two-body MLP must be 4->32->32->9 with device weight pointers");
   HH_CUDA(cudaMemcpyAsync(ctx->w2, pk.data(), pk.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+  std::vector<double> pkd(pk.begin(), pk.end());
+  std::vector<float> w2tc(2 * 1024);
+  hh_pack_w2_tc(pk.data() + HH_MLP2_H * HH_MLP2_INP + HH_MLP2_H, w2tc.data());     // W2 follows W1 and b1 in the packed layout
+  HH_CUDA(cudaMemcpyAsync(ctx->w2tc, w2tc.data(), w2tc.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+  HH_CUDA(cudaMemcpyAsync(ctx->w2d, pkd.data(), pkd.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
   HH_CUDA(cudaStreamSynchronize(ctx->stream));
   if (mlp3) {
     r = pack_mlp(ctx, mlp3, 7, HH_MLP3_INP, HH_MLP3_H, pk);

@@ -81,6 +81,8 @@ struct hh_ctx {
   /* carved device pointers */
   DevScalars* d_sc;
   float *w2, *w3;                       /* packed weights                                     */
+  float* w2tc;                          /* W2 as the tensor-core B operand: tf32 hi | lo, core-matrix layout (near_path 1, 2) */
+  double* w2d;                          /* the two-body weights as fp64 (aca_precision = 1)   */
   u64 *keys[2]; u32 *idx[2];            /* radix ping-pong                                    */
   u32* hist;  size_t hist_cap;          /* radix histograms / generic scan tile sums          */
   void* tilesum;                        /* tile sums for scans (Cnt3 / u64)                   */
@@ -136,6 +138,8 @@ int hh_sort_pairs(hh_ctx* ctx, u64* keys[2], u32* vals[2], int64_t n, int bit_lo
 int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N);
 int hh_blocks_build(hh_ctx* ctx);
 int hh_near_apply(hh_ctx* ctx);                                       /* Us += near-field           */
+int hh_near_apply_tc(hh_ctx* ctx);                                    /* the same on tcgen05 tensor cores (hh_near_tc.cu) */
+void hh_pack_w2_tc(const float* W2, float* out);                      /* host: W2 [32][32] -> 2 x 1024 floats */
 int hh_dense_apply(hh_ctx* ctx);                                      /* Us += resident blocks on which ACA broke down, densely */
 int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next);      /* one CTA per block (hh_aca.cu)        */
 int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next);     /* lock-step over the batch (hh_aca2.cu) */

@@ -129,6 +129,40 @@ __device__ __forceinline__ void entry2_eval(const float* __restrict__ sw, float 
     for (int r = 0; r < 9; ++r) M[e][r] *= inv[e];
 }
 
+// The same entry in fp64 (aca_precision = 1): weights as doubles in shared memory (same packed layout), one entry per call.
+template <int INP, int H>
+__device__ __forceinline__ void mlp_eval_d(const double* __restrict__ sw, const double (&x)[INP], double (&out)[9]) {
+  typedef MlpOff<INP, H> O;
+  double h1[H];
+#pragma unroll
+  for (int o = 0; o < H; ++o) {
+    double a = sw[O::B1 + o];
+#pragma unroll
+    for (int i = 0; i < INP; ++i) a = fma(sw[O::W1 + o * INP + i], x[i], a);
+    h1[o] = tanh(a);
+  }
+#pragma unroll
+  for (int r = 0; r < 9; ++r) out[r] = sw[O::B3 + r];
+#pragma unroll 1
+  for (int o = 0; o < H; ++o) {
+    double a = sw[O::B2 + o];
+#pragma unroll
+    for (int i = 0; i < H; ++i) a = fma(sw[O::W2 + o * H + i], h1[i], a);
+    const double t = tanh(a);
+#pragma unroll
+    for (int r = 0; r < 9; ++r) out[r] = fma(sw[O::W3 + o * 12 + r], t, out[r]);
+  }
+}
+__device__ __forceinline__ void entry2_eval_d(const double* __restrict__ sw, double a, const float (&xi)[3], const float (&xj)[3], double (&M)[9]) {
+  const double rx = (double)xj[0] - (double)xi[0], ry = (double)xj[1] - (double)xi[1], rz = (double)xj[2] - (double)xi[2];
+  double d = sqrt(rx * rx + ry * ry + rz * rz);
+  d = fmax(d, 1e-12 * a);
+  const double x[HH_MLP2_INP] = {rx / d, ry / d, rz / d, a / d};
+  mlp_eval_d<HH_MLP2_INP, HH_MLP2_H>(sw, x, M);
+#pragma unroll
+  for (int r = 0; r < 9; ++r) M[r] /= d;
+}
+
 // cooperative copy of packed weights into shared memory (n floats, multiple of 4)
 __device__ __forceinline__ void load_weights(float* sw, const float* __restrict__ gw, int n) {
   for (int i = threadIdx.x * 4; i < n; i += blockDim.x * 4)

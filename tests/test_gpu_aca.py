@@ -94,20 +94,23 @@ def test_block_factors_vs_oracle_replay(rule, mlp2):
 # bound the replay parity"): the plain rows report what fp32 entries achieve on the listing as printed and assert the
 # north_star bar where it is met; S-18b (opt-in, kappa > 0: ill-conditioned pivots break Alg. 2 down, the block is
 # applied densely) is what brings ball / chain clouds inside 1e-5.  BARS[name] = (bar on U, bar on the far-field part).
+#   *_f64: aca_precision = 1 (fp64 entries and residuals in Alg. 2, factors still fp32), plain listing: the discrepancy is gone.
 CASES = [
-    ("c1", lambda: synth.cube_cloud(2048, 0.1), 64, 1.0, 1e-4, 0.0),
-    ("cube_leaf16_eta2", lambda: synth.cube_cloud(4000, 0.1), 16, 2.0, 1e-3, 0.0),
-    ("ball_1e-5", lambda: synth.ball_cloud(5000, 0.2), 32, 1.0, 1e-5, 0.0),
-    ("ball_1e-5_S18b", lambda: synth.ball_cloud(5000, 0.2), 32, 1.0, 1e-5, 300.0),
-    ("chains", lambda: synth.chain_cloud(120, 50, 0.1), 32, 1.0, 1e-4, 0.0),
-    ("chains_S18b", lambda: synth.chain_cloud(120, 50, 0.1), 32, 1.0, 1e-4, 50.0),
+    ("c1", lambda: synth.cube_cloud(2048, 0.1), 64, 1.0, 1e-4, 0.0, 0),
+    ("cube_leaf16_eta2", lambda: synth.cube_cloud(4000, 0.1), 16, 2.0, 1e-3, 0.0, 0),
+    ("ball_1e-5", lambda: synth.ball_cloud(5000, 0.2), 32, 1.0, 1e-5, 0.0, 0),
+    ("ball_1e-5_S18b", lambda: synth.ball_cloud(5000, 0.2), 32, 1.0, 1e-5, 300.0, 0),
+    ("ball_1e-5_f64", lambda: synth.ball_cloud(5000, 0.2), 32, 1.0, 1e-5, 0.0, 1),
+    ("chains", lambda: synth.chain_cloud(120, 50, 0.1), 32, 1.0, 1e-4, 0.0, 0),
+    ("chains_S18b", lambda: synth.chain_cloud(120, 50, 0.1), 32, 1.0, 1e-4, 50.0, 0),
+    ("chains_f64", lambda: synth.chain_cloud(120, 50, 0.1), 32, 1.0, 1e-4, 0.0, 1),
 ]
-BARS = {"c1": (1e-5, 1e-5), "cube_leaf16_eta2": (1e-5, 1e-5), "ball_1e-5": (1e-4, 2e-4), "ball_1e-5_S18b": (1e-5, 3e-5),
-        "chains": (1e-4, 2e-4), "chains_S18b": (1e-5, 1e-5)}
+BARS = {"c1": (1e-5, 1e-5), "cube_leaf16_eta2": (1e-5, 1e-5), "ball_1e-5": (1e-5, 3e-5), "ball_1e-5_S18b": (1e-5, 3e-5),
+        "ball_1e-5_f64": (1e-5, 1e-5), "chains": (3e-5, 1e-4), "chains_S18b": (1e-5, 1e-5), "chains_f64": (1e-5, 1e-5)}
 
 
-@pytest.mark.parametrize("name,gen,leaf,eta,zeta,kappa", CASES)
-def test_matvec_vs_oracle(name, gen, leaf, eta, zeta, kappa, mlp2):
+@pytest.mark.parametrize("name,gen,leaf,eta,zeta,kappa,prec", CASES)
+def test_matvec_vs_oracle(name, gen, leaf, eta, zeta, kappa, prec, mlp2):
     X = gen()
     N = len(X)
     F = synth.gaussian_forces(N)
@@ -115,7 +118,7 @@ def test_matvec_vs_oracle(name, gen, leaf, eta, zeta, kappa, mlp2):
     H = oracle.HMatrix(X, mlp2, leaf=leaf, eta=f32(eta))
     H.set_replay_roundoff(2.0 ** -24)
     H.set_kappa_max(kappa if kappa > 0 else float("inf"))
-    ctx = setup(X, mlp2, leaf_size=leaf, eta=eta, aca_tol=zeta, kappa_max=kappa, ws_mb=8192)
+    ctx = setup(X, mlp2, leaf_size=leaf, eta=eta, aca_tol=zeta, kappa_max=kappa, aca_precision=prec, ws_mb=8192)
     U = ctx.matvec(to_dev(F)).cpu().numpy()
     tr = ctx.get_tree()
     st = ctx.stats()
@@ -134,7 +137,11 @@ def test_matvec_vs_oracle(name, gen, leaf, eta, zeta, kappa, mlp2):
     assert err_far <= bar_far
     if kappa == 0.0:
         # plain listing: flag 2 can only be an exactly singular pivot (|det| < 1e-30, S-18)
-        assert np.array_equal(info["flags"], flags)
+        diff = np.flatnonzero(info["flags"] != flags)
+        for g in diff[:8]:
+            print(name, "flag mismatch: oracle block", g, "shape", H.block_shape(int(g)), "GPU flag", flags[g], "replay flag", info["flags"][g],
+                  "rank", replay[0][g])
+        assert len(diff) <= info["replay_bad"] and len(diff) <= 2, "plain listing: only an exactly singular pivot may change a flag"
     else:
         # S-18b: the replay takes the GPU's breakdowns as given and judges them (plausible within a factor 2 of kappa);
         # a flag differs only where the fp64 replay meets an exactly singular pivot that fp32 noise hid from the GPU,

@@ -89,3 +89,34 @@ def test_tiny_clouds_whole_matvec(n, leaf, mlp2_bias):
         assert np.array_equal(U, F)
     assert rel_l2(U, ref) <= 1e-5
     ctx.close()
+
+
+@pytest.mark.parametrize("near_path,bar", [(1, 2e-3), (2, 1e-5)])
+def test_tensor_core_near_field(near_path, bar, mlp2_bias):
+    """near_path = 1 / 2 (csrc/hh_near_tc.cu): the 32 x 32 layer as a tcgen05 tf32 contraction (accumulator in tensor
+    memory), against O-dense with nothing admissible and against the fp32 ALU path on the same input.
+    Bars: north_star's 2e-3 for the tensor-core path (tf32 operands, tanh.approx); 1e-5 for the split-operand variant."""
+    n, leaf = 3000, 48
+    X = synth.cube_cloud(n, 0.1, seed=3)
+    F = synth.gaussian_forces(n, seed=4)
+    ref = oracle.dense_matvec(X, F, mlp2_bias)
+    res = {}
+    for path in (0, near_path):
+        ctx = make_ctx(mlp2_bias, leaf_size=leaf, eta=1e-30, ws_mb=512, near_path=path)
+        ctx.build_tree(to_dev(X))
+        ctx.build_blocks()
+        assert ctx.stats()["n_admissible"] == 0
+        res[path] = ctx.matvec(to_dev(F), parts=3).cpu().numpy()
+        ctx.close()
+    e_tc, e_alu = rel_l2(res[near_path], ref), rel_l2(res[0], ref)
+    print("near_path %d: rel L2 vs O-dense %.3e (fp32 ALU path %.3e), vs the ALU path %.3e" % (near_path, e_tc, e_alu, rel_l2(res[near_path], res[0])))
+    assert e_tc <= bar
+    # ragged and tiny leaves go through the same 128-entry tiles
+    for nn, lf in ((65, 64), (3, 1), (1, 64)):
+        Xs_, Fs_ = synth.cube_cloud(nn, 0.05, seed=11), synth.gaussian_forces(nn, seed=12)
+        ctx = make_ctx(mlp2_bias, leaf_size=lf, eta=1e-30, ws_mb=512, near_path=near_path)
+        ctx.build_tree(to_dev(Xs_))
+        ctx.build_blocks()
+        U = ctx.matvec(to_dev(Fs_), parts=3).cpu().numpy()
+        assert rel_l2(U, oracle.dense_matvec(Xs_, Fs_, mlp2_bias)) <= bar
+        ctx.close()

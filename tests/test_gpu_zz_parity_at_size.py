@@ -77,7 +77,7 @@ def capture_to_replay(rec, omap, nG):
     return (rr, np.ascontiguousarray(rec[:, 4:100][sel], np.int32), np.ascontiguousarray(rec[:, 100:196][sel], np.int32), rf), og
 
 
-def parity_at_size(name, X, F, mlp2, leaf, eta, zeta, kappa, runs, run_len, n_dense, size_cap=None, H=None, ctx=None, bar=1e-5):
+def parity_at_size(name, X, F, mlp2, leaf, eta, zeta, kappa, runs, run_len, n_dense, size_cap=None, H=None, ctx=None, bar=1e-5, prec=0):
     """GPU two-body mat-vec (self + near + far) vs the oracle on sampled tree-order runs.  size_cap: only admissible blocks
     with max(|tau|,|sigma|) <= size_cap take part on both sides (the far-field is then accumulated batch by batch through
     hh_aca + hh_far_apply_resident, the same kernels)."""
@@ -87,11 +87,12 @@ def parity_at_size(name, X, F, mlp2, leaf, eta, zeta, kappa, runs, run_len, n_de
     if H is None:
         H = oracle.HMatrix(X, mlp2, leaf=leaf, eta=f32(eta))
     H.set_kappa_max(kappa if kappa > 0 else float("inf"))
+    H.set_replay_roundoff(2.0 ** -24)       # decisions are judged up to the fp32 rounding of the replayed arithmetic
     own = ctx is None
     if own:
-        ctx = make_ctx(mlp2, ws_mb=_ws_mb(), leaf_size=leaf, eta=eta, aca_tol=zeta, kappa_max=kappa)
+        ctx = make_ctx(mlp2, ws_mb=_ws_mb(), leaf_size=leaf, eta=eta, aca_tol=zeta, kappa_max=kappa, aca_precision=prec)
     else:
-        ctx.set_params(eta=eta, aca_tol=zeta, kappa_max=kappa)
+        ctx.set_params(eta=eta, aca_tol=zeta, kappa_max=kappa, aca_precision=prec)
     ctx.build_tree(to_dev(X))
     ctx.build_blocks()
     tr = ctx.get_tree()
@@ -141,10 +142,10 @@ def parity_at_size(name, X, F, mlp2, leaf, eta, zeta, kappa, runs, run_len, n_de
     ndense_blocks = int((replay[3] == 2).sum())
     # flags of the replay: equal, except blocks where the fp64 replay meets an exactly singular pivot (S-18)
     fl_diff = np.flatnonzero(info["flags"][og] != replay[3][og])
-    print("%s: N=%d leaf=%d eta=%g zeta=%g kappa=%s | %d rows in %d runs, %d target leaves, %d blocks replayed (%d dense), "
+    print("%s: N=%d leaf=%d eta=%g zeta=%g kappa=%s aca_precision=%d | %d rows in %d runs, %d target leaves, %d blocks replayed (%d dense), "
           "oracle entries %.3e in %.0f s (%d threads), GPU side %.0f s | rel L2 GPU vs replay = %.3e | decisions outside slack %d, "
           "outside slack+rounding %d of %d | flag mismatches %d"
-          % (name, N, leaf, eta, zeta, kappa if kappa > 0 else "inf", len(rows), runs, leaves_hit, n_rec, ndense_blocks, info["entries"],
+          % (name, N, leaf, eta, zeta, kappa if kappa > 0 else "inf", prec, len(rows), runs, leaves_hit, n_rec, ndense_blocks, info["entries"],
              t_orc, oracle.num_threads(), t_gpu, err, nstrict, nbad, int(3 * replay[0].sum()), len(fl_diff)))
     out = dict(err=err, leaves=leaves_hit, info=info, st=st, blocks=n_rec)
     if n_dense > 0:
@@ -160,10 +161,13 @@ def parity_at_size(name, X, F, mlp2, leaf, eta, zeta, kappa, runs, run_len, n_de
             print("%s: eps_r on %d particles vs O-dense (%.0f s): GPU %.3e, fp64 replay with the same pivots %.3e (zeta %g)"
                   % (name, len(pick), time.time() - t2, eg, eo, zeta))
             out.update(eps_gpu=eg, eps_orc=eo)
-    assert err <= bar, "GPU vs oracle replay on sampled target leaves"
-    assert len(fl_diff) <= nbad
+    out.update(nbad=nbad, fl_diff=len(fl_diff))
     if own:
         ctx.close()
+    if os.environ.get("HH_PARITY_REPORT_ONLY", "0") == "1":
+        return out
+    assert err <= bar, "GPU vs oracle replay on sampled target leaves"
+    assert len(fl_diff) <= nbad
     return out
 
 
@@ -174,8 +178,11 @@ def env_int(name, default):
 def test_c3_replay_on_sampled_leaves_and_dense(mlp2):
     """c3 as bench.py times it (eta 1, zeta 1e-4, plain listing): >= 256 sampled target leaves, >= 1000 dense rows"""
     cfg, X, F = synth.config("c3")
-    r = parity_at_size("c3", X, F, mlp2, cfg["leaf"], cfg["eta"], cfg["tol"], float(cfg.get("kappa_max", 0.0)),
-                       runs=env_int("HH_PARITY_RUNS", 2), run_len=6144, n_dense=env_int("HH_PARITY_DENSE", 1000))
+    r = parity_at_size("c3", X, F, mlp2, cfg["leaf"], cfg["eta"], cfg["tol"], float(os.environ.get("HH_PARITY_KAPPA", cfg.get("kappa_max", 0.0))),
+                       runs=env_int("HH_PARITY_RUNS", 2), run_len=6144, n_dense=env_int("HH_PARITY_DENSE", 1000),
+                       prec=env_int("HH_PARITY_PREC", 0), size_cap=env_int("HH_PARITY_CAP", 0) or None)
+    if os.environ.get("HH_PARITY_REPORT_ONLY", "0") == "1":
+        return
     assert r["leaves"] >= 256 and r["st"]["aca_batches"] >= 2
     # Eq. (11): the H mat-vec is as close to O-dense as Alg. 2 in fp64 with the same pivots is; zeta itself is a heuristic
     # bound (L205, L283: "effective upper bound"), asserted with the factor the fp64 run needs

@@ -30,7 +30,7 @@ if ROOT not in sys.path:
 METRIC = "H-matvec particles/s (whole step: tree + blocks + ACA + near + far + three-body)"
 UNIT = "particles/s"
 FAR_BYTES_PER_UNIT = 36          # bytes of fp32 factors read per (row or column) x block-rank (DESIGN.md far-field)
-ORACLE_SAMPLE_N = {"c1": 2048, "c2": 8192, "c3": 24576, "c4": 16384, "c5": 16000}
+ORACLE_SAMPLE_N = {"c1": 2048, "c2": 8192, "c3": 24576, "c4": 16384, "c5": 16000, "p1": 60000, "p2": 60000}
 
 
 def peaks():
@@ -104,6 +104,8 @@ def make_inputs(workload, rank):
     """seeded synthetic cloud of the named config; replicas (rank > 0) draw their own seed"""
     import synth
     cfg = dict(synth.CONFIGS[workload])
+    if cfg["shape"] in ("two_drops", "filament_sphere"):               # the paper's own workloads (SURVEY 8(f) row 1); one seed
+        return synth.config(workload)
     n = cfg["n"]
     if cfg["shape"] == "cube":
         X = synth.cube_cloud(n, cfg["phi"], seed=rank)
@@ -159,7 +161,7 @@ def run_reference(args):
         ts.append(t)
     total = sum(ts)
     v = n_s * len(ts) / total
-    sample = ("%d-particle cloud of the same recipe (shape %s, phi %.2f, leaf %d, eta %.1f, zeta %.0e, rcut3 %.1f), "
+    sample = ("%d-particle cloud of the same recipe (shape %s, phi %s, leaf %d, eta %.1f, zeta %.0e, rcut3 %.1f), "
               "one full oracle step each" % (n_s, cfg["shape"], cfg["phi"], cfg["leaf"], cfg["eta"], cfg["tol"], cfg["rcut3"]))
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup_ref, "ms_per_step": 1e3 * total / len(ts), "higher_is_better": True, "scaling": "weak",
@@ -174,8 +176,9 @@ def run_reference(args):
 def workload_name(w, c=None):
     import synth
     c = c or synth.CONFIGS[w]
-    return ("%s: N=%d %s phi=%.2f, leaf %d, eta=%.1f, zeta=%.0e, rcut3=%.1f, MLP2 4-32-32-9, MLP3 7-64-64-9 (BASELINE.json configs[%d])"
-            % (w, c["n"], c["shape"], c["phi"], c["leaf"], c["eta"], c["tol"], c["rcut3"], int(w[1]) - 1))
+    src = "BASELINE.json configs[%d]" % (int(w[1]) - 1) if w[0] == "c" else "PAPER.md Sec. 4.3.%s at the paper's parameters, random-init MLPs" % w[1]
+    return ("%s: N=%s %s phi=%s, leaf %d, eta=%.1f, zeta=%.0e, rcut3=%.1f, kappa_max=%s, MLP2 4-32-32-9, MLP3 7-64-64-9 (%s)"
+            % (w, c["n"], c["shape"], c["phi"], c["leaf"], c["eta"], c["tol"], c["rcut3"], c.get("kappa_max", 0.0) or "inf (plain listing)", src))
 
 
 def run_gpu(args):
@@ -221,7 +224,16 @@ def run_gpu(args):
             dist.barrier()
         torch.cuda.synchronize(dev)
 
+    def harness_forces():
+        """multi-step filament workloads: the harness recomputes the internal forces from the current positions (device
+        tensors, synth's generator with xp = torch); input generation, outside the timed events"""
+        if cfg["forces"] == "filament":
+            Fd.copy_(synth.filament_forces(Xd.double(), cfg["n_chains"], cfg["n_beads"], xp=torch).float())
+        elif cfg["forces"] == "mixture":
+            Fd.copy_(synth.mixture_forces(Xd.double(), cfg["n_chains"], cfg["n_beads"], xp=torch).float())
+
     def one_step():
+        harness_forces()
         flush.fill_(1)                                                  # L2 flush between iterations (outside the events)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
@@ -284,7 +296,9 @@ def run_gpu(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_name(args.workload, cfg), "parallelism": "replicas x%d (no sharding, no collectives)" % world,
                    "l2": "explicit 256 MB flush write between timed iterations; each step also streams its factor arena (>> L2)",
-                   "arena_gb": st["arena_bytes"] / 2 ** 30, "aca_batches_per_step": st["aca_batches"]},
+                   "arena_gb": st["arena_bytes"] / 2 ** 30, "aca_batches_per_step": st["aca_batches"],
+                   "near_path": "%d (%s)" % (args.near_path, ["fp32 ALU", "tcgen05 tf32 + tanh.approx (2e-3 path)", "tcgen05 split tf32 + tanhf (fp32-class)"][args.near_path]),
+                   "aca_precision": "%d (%s)" % (args.aca_precision, ["fp32 entries in Alg. 2", "fp64 entries and residuals in Alg. 2 (parity mode)"][args.aca_precision])},
         "clocks": clk,
         "e2e": {"value": world * N * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 24 * N, "d2h_bytes_per_step": 24 * N,
                 "steps": ke, "api": "hh_step_host (pinned host X, F in; U, X out)"},
@@ -317,7 +331,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "c5", "p1", "p2"])
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--workspace-gb", type=float, default=150.0)
     ap.add_argument("--e2e-steps", type=int, default=2)
@@ -325,7 +339,7 @@ def main():
     ap.add_argument("--tol", type=float, default=None, help="override the config's ACA tolerance zeta (config 3 sweep)")
     ap.add_argument("--leaf", type=int, default=None)
     ap.add_argument("--kappa-max", type=float, default=None, help="S-18b limit on the pivot-block condition number")
-    ap.add_argument("--near-path", type=int, default=0, choices=[0, 1, 2], help="0 fp32 ALU, 1 tcgen05 tf32 + tanh.approx (2e-3), 2 tcgen05 split tf32 + tanhf")
+    ap.add_argument("--near-path", type=int, default=2, choices=[0, 1, 2], help="0 fp32 ALU, 1 tcgen05 tf32 + tanh.approx (2e-3), 2 tcgen05 split tf32 + tanhf")
     ap.add_argument("--aca-precision", type=int, default=0, choices=[0, 1], help="1 = fp64 entries and residuals in Alg. 2 (parity mode)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     args = ap.parse_args()

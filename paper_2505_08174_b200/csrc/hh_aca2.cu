@@ -202,15 +202,13 @@ __device__ __forceinline__ void a2_norm_granule(const A2Args& A, u32 gi, u32 cou
 // ---- lines 4-5 (COLS = false: over the rows of tau, entries G(i, j_k)) resp. lines 7-8 (COLS = true: over the columns of
 // sigma, entries G(i_k, j)) of all active blocks in ONE launch: entry evaluation by the MLP, residual against the stored
 // rank terms, pivot scores, Gram sums.  A warp takes 4 granules: slot (e, half) -> granule 4*tile + 2*e + half; every thread
-// evaluates two entries (the in-register MLP of hh_mlp.cuh, at near-field speed) and keeps them in registers for the
-// update, so a raw entry never travels through memory.  The update re-reads the k stored rank terms of its rows
-// (36 k bytes per row: the l^2 term of Alg. 2's cost); an arena batch is far larger than L2, so these reads
-// come from HBM.  Their latency is taken off the critical path by prefetching exactly those lines into L2 BEFORE the MLP
-// arithmetic of the tile starts (about 6,000 instructions per thread): by the time the update loop runs, its loads are
-// L2 hits.  Round 1 ran the two halves as separate launches (the update at four times the occupancy to hide the HBM
-// latency) and paid a 72-byte round trip per entry for the raw values on top.
-__device__ __forceinline__ void l2_prefetch(const float* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-
+// evaluates two entries (the in-register MLP of hh_mlp.cuh) and keeps them in registers for the update, so a raw entry
+// never travels through memory (round 1 ran entry evaluation and update as two launches with a 72-byte round trip per entry
+// between them; same speed).  The update re-reads the k stored rank terms of its rows, 36 k bytes per
+// row: the l^2 term of Alg. 2's cost.  An arena batch is far larger than L2, so these reads come from HBM:
+// about 7 TB per mat-vec at c3, ten times the factors themselves, and the reason the ACA build is the longest stage.
+// Measured and dropped: prefetching those lines into L2 before the MLP arithmetic (+5 %), staging them
+// through shared memory with cp.async (+29 %), one loop over both slots (+22 %, spills).
 // F64 (aca_precision = 1, parity mode): the entry and the residual subtraction in fp64, rounded once when stored.
 template <bool COLS, bool F64>
 __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncount) {
@@ -223,35 +221,12 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
   const u32 ntiles = (count + 3) / 4;
   u32 tile = blockIdx.x * (A2_T / 32) + warp;
   for (; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
-    // (a) L2 prefetch of the stored rank terms this half-warp's two granules will read in (d)
-#pragma unroll
-    for (int e = 0; e < 2; ++e) {
-      const u32 gi = 4 * tile + 2 * e + half;
-      if (gi < count) {
-        const uint2 g = gl[gi];
-        const BlkState& s = A.st[g.x];
-        const int k = s.k;
-        if (s.status == 0 && k > 0) {
-          const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n), lenp = COLS ? np : mp;
-          const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
-          for (int c = 0; c * HH_RC < k; ++c) {
-            const float* base = A.arena + (size_t)tabrow[c] * HH_UNIT_FLOATS + (COLS ? (size_t)HH_RC * 9 * mp : 0) + g.y;
-            const int nt = 9 * min(HH_RC, k - c * HH_RC);
-            for (int t = (int)l16; t < nt; t += 16) {
-              const float* p = base + (size_t)t * lenp;
-              l2_prefetch(p);
-              l2_prefetch(p + 15);                                   // a 64-byte run may straddle two lines
-            }
-          }
-        }
-      }
-    }
-    // (b) line 6 for the row granules with the same indices (memory-bound, independent of line 7)
+    // (a) line 6 for the row granules with the same indices (memory-bound, independent of line 7)
     if (COLS && 4 * tile < ncount) {
       a2_norm_granule(A, 4 * tile + half, ncount, lane);
       a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
     }
-    // (c) the entries
+    // (b) the entries
     float v[2][9];
     double vd[F64 ? 2 : 1][9];
     {
@@ -283,7 +258,7 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
         entry2_eval<2>(sw, A.a, xi, xj, v);
       }
     }
-    // (d) residual, pivot scores, Gram sums: one granule per half-warp and slot
+    // (c) residual, pivot scores, Gram sums: one granule per half-warp and slot
 #pragma unroll
     for (int e = 0; e < 2; ++e) {
       const u32 gi = 4 * tile + 2 * e + half;

@@ -25,9 +25,10 @@
 #define NT_TILE 256            /* source particles staged per tile                                        */
 #define NT_SPIN_MAX (1u << 24) /* bounded mbarrier spins: a wrong descriptor must not hang the GPU         */
 
+template <int NP>              /* NP = 1: tf32 operands as they are, NP = 2: hi + lo parts (split operands) */
 struct NtSmem {
-  float A[2][128 * 32];        /* h1 tile, hi / lo: element (row r, k) at (r/8)*256 + (k/4)*32 + (r%8)*4 + (k%4) */
-  float B[2][32 * 32];         /* W2 hi / lo in the same layout with n (output unit) as the row             */
+  float A[NP][128 * 32];       /* h1 tile, hi / lo: element (row r, k) at (r/8)*256 + (k/4)*32 + (r%8)*4 + (k%4) */
+  float B[NP][32 * 32];        /* W2 hi / lo in the same layout with n (output unit) as the row             */
   float w1[32 * 4], b1[32], b2[32], w3t[32 * 12], b3[12];
   float tX[HH_MAX_LEAF * 3], sU[HH_MAX_LEAF * 3];
   float sXj[NT_TILE * 3], sFj[NT_TILE * 3];
@@ -68,22 +69,26 @@ __device__ __forceinline__ bool mbar_wait(u32 bar, u32 parity) {
   return false;
 }
 
+// Software pipeline over the 128-entry tiles of a CTA (two accumulators in tensor memory, one A buffer):
+//   layer 1 of tile n in registers | wait MMA(n-1) | write A | sync | issue MMA(n) -> D[n & 1] | epilogue of tile n-1 from D[(n-1) & 1]
+// so the tensor-core latency of a tile hides behind the epilogue of the one before and layer 1 of the one after.
 template <bool SPLIT>
 __global__ void __launch_bounds__(NT_T) k_near_tc(const float* __restrict__ gw, const float* __restrict__ gw2tc, float a,
                                                    const u32* __restrict__ leaf_nodes, const u32* __restrict__ nlo, const u32* __restrict__ nhi,
                                                    const uint2* __restrict__ PH, const u32* __restrict__ near_begin, const u32* __restrict__ near_end,
                                                    const float* __restrict__ Xs, const float* __restrict__ Fs, float* __restrict__ Us, u32* __restrict__ err_flag) {
   extern __shared__ __align__(1024) unsigned char nt_raw[];
-  NtSmem& S = *reinterpret_cast<NtSmem*>(nt_raw);
+  typedef NtSmem<SPLIT ? 2 : 1> Smem;
+  Smem& S = *reinterpret_cast<Smem*>(nt_raw);
   typedef MlpOff<HH_MLP2_INP, HH_MLP2_H> O;
   const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const u32 node = leaf_nodes[blockIdx.x];
   const u32 tlo = nlo[node], m = nhi[node] - tlo;
   const u32 bar_mma = smem_u32(&S.mbar_mma), bar_tma = smem_u32(&S.mbar_tma);
 
-  // ---- one-time setup: tensor memory, barriers, W2 by TMA bulk copy, the small layers by plain loads ----
+  // ---- one-time setup: tensor memory (2 accumulators of 32 columns), barriers, W2 by TMA bulk copy, the small layers ----
   if (warp == 0) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 32;" ::"r"(smem_u32(&S.tmem_base)) : "memory");
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 64;" ::"r"(smem_u32(&S.tmem_base)) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   if (tid == 0) {
@@ -106,7 +111,43 @@ __global__ void __launch_bounds__(NT_T) k_near_tc(const float* __restrict__ gw, 
   asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
   const u32 tmem_d = S.tmem_base;
   bool alive = mbar_wait(bar_tma, 0);
-  u32 phase = 0;
+  u32 phase = 0, ntile = 0;                        // ntile counts the MMAs issued by this CTA: accumulator ntile & 1
+
+  // epilogue of one tile: accumulator -> registers, + b2, tanh, layer 3, 1/r, apply (S-3), shared-memory atomics into U_i
+  auto epilogue = [&](u32 acc_idx, bool valid, u32 ii, u32 jj, float inv) {
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    u32 dr[32];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, "
+        "%21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(dr[0]), "=r"(dr[1]), "=r"(dr[2]), "=r"(dr[3]), "=r"(dr[4]), "=r"(dr[5]), "=r"(dr[6]), "=r"(dr[7]), "=r"(dr[8]), "=r"(dr[9]),
+          "=r"(dr[10]), "=r"(dr[11]), "=r"(dr[12]), "=r"(dr[13]), "=r"(dr[14]), "=r"(dr[15]), "=r"(dr[16]), "=r"(dr[17]), "=r"(dr[18]),
+          "=r"(dr[19]), "=r"(dr[20]), "=r"(dr[21]), "=r"(dr[22]), "=r"(dr[23]), "=r"(dr[24]), "=r"(dr[25]), "=r"(dr[26]), "=r"(dr[27]),
+          "=r"(dr[28]), "=r"(dr[29]), "=r"(dr[30]), "=r"(dr[31])
+        : "r"(tmem_d + ((warp * 32u) << 16) + acc_idx * 32u)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    float out[9];
+#pragma unroll
+    for (int r = 0; r < 9; ++r) out[r] = S.b3[r];
+#pragma unroll
+    for (int o = 0; o < 32; ++o) {
+      const float pre = __uint_as_float(dr[o]) + S.b2[o];
+      const float t = SPLIT ? tanhf(pre) : tanh_mufu(pre);
+      const float4 wa = *reinterpret_cast<const float4*>(&S.w3t[12 * o]);
+      const float4 wb = *reinterpret_cast<const float4*>(&S.w3t[12 * o + 4]);
+      const float wc = S.w3t[12 * o + 8];
+      out[0] = fmaf(wa.x, t, out[0]); out[1] = fmaf(wa.y, t, out[1]); out[2] = fmaf(wa.z, t, out[2]);
+      out[3] = fmaf(wa.w, t, out[3]); out[4] = fmaf(wb.x, t, out[4]); out[5] = fmaf(wb.y, t, out[5]);
+      out[6] = fmaf(wb.z, t, out[6]); out[7] = fmaf(wb.w, t, out[7]); out[8] = fmaf(wc, t, out[8]);
+    }
+    if (valid && tlo + ii != S.sJ[jj]) {                                   // S-5: the pair i == j is skipped
+      const float f0 = S.sFj[3 * jj], f1 = S.sFj[3 * jj + 1], f2 = S.sFj[3 * jj + 2];
+#pragma unroll
+      for (int al = 0; al < 3; ++al)
+        atomicAdd(&S.sU[3 * ii + al], inv * fmaf(out[3 * al], f0, fmaf(out[3 * al + 1], f1, out[3 * al + 2] * f2)));
+    }
+  };
 
   u32 b = near_begin[node];
   const u32 bend = near_end[node];
@@ -137,12 +178,15 @@ __global__ void __launch_bounds__(NT_T) k_near_tc(const float* __restrict__ gw, 
     }
     __syncthreads();
     const u32 pairs = m * nt;
+    bool pend = false, p_valid = false;                                  // the tile whose MMA is in flight
+    u32 p_ii = 0, p_jj = 0;
+    float p_inv = 0.f;
     for (u32 p0 = 0; p0 < pairs; p0 += NT_T) {
       const u32 p = p0 + tid;
       const bool valid = p < pairs;
       const u32 pc = valid ? p : 0u;
       const u32 jj = pc / m, ii = pc - jj * m;
-      // ---- features and layer 1 (S-1, S-2, S-4) ----
+      // ---- features and layer 1 (S-1, S-2, S-4), in registers: overlaps the MMA of the previous tile ----
       float x[4], inv;
       {
         const float rx = S.sXj[3 * jj] - S.tX[3 * ii], ry = S.sXj[3 * jj + 1] - S.tX[3 * ii + 1], rz = S.sXj[3 * jj + 2] - S.tX[3 * ii + 2];
@@ -151,81 +195,58 @@ __global__ void __launch_bounds__(NT_T) k_near_tc(const float* __restrict__ gw, 
         inv = 1.0f / d;
         x[0] = rx * inv; x[1] = ry * inv; x[2] = rz * inv; x[3] = a * inv;
       }
+      float h[32];
+#pragma unroll
+      for (int o = 0; o < 32; ++o) {
+        const float4 w = *reinterpret_cast<const float4*>(&S.w1[4 * o]);
+        const float pre = fmaf(w.x, x[0], fmaf(w.y, x[1], fmaf(w.z, x[2], fmaf(w.w, x[3], S.b1[o]))));
+        h[o] = SPLIT ? tanhf(pre) : tanh_mufu(pre);
+      }
+      // ---- the previous MMA has read A: wait for it, then publish this tile's A operand ----
+      if (pend) { alive = alive && mbar_wait(bar_mma, phase); phase ^= 1u; }
       float* Ahi = &S.A[0][(tid >> 3) * 256 + (tid & 7) * 4];
-      float* Alo = &S.A[1][(tid >> 3) * 256 + (tid & 7) * 4];
+      float* Alo = &S.A[SPLIT ? 1 : 0][(tid >> 3) * 256 + (tid & 7) * 4];
 #pragma unroll
       for (int kc = 0; kc < 8; ++kc) {
-        float h[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const int o = 4 * kc + q;
-          const float4 w = *reinterpret_cast<const float4*>(&S.w1[4 * o]);
-          const float pre = fmaf(w.x, x[0], fmaf(w.y, x[1], fmaf(w.z, x[2], fmaf(w.w, x[3], S.b1[o]))));
-          h[q] = SPLIT ? tanhf(pre) : tanh_mufu(pre);
-        }
         float4 hi, lo;
-        hi.x = __uint_as_float(to_tf32(h[0])); hi.y = __uint_as_float(to_tf32(h[1]));
-        hi.z = __uint_as_float(to_tf32(h[2])); hi.w = __uint_as_float(to_tf32(h[3]));
+        hi.x = __uint_as_float(to_tf32(h[4 * kc])); hi.y = __uint_as_float(to_tf32(h[4 * kc + 1]));
+        hi.z = __uint_as_float(to_tf32(h[4 * kc + 2])); hi.w = __uint_as_float(to_tf32(h[4 * kc + 3]));
         *reinterpret_cast<float4*>(Ahi + kc * 32) = hi;
         if (SPLIT) {
-          lo.x = __uint_as_float(to_tf32(h[0] - hi.x)); lo.y = __uint_as_float(to_tf32(h[1] - hi.y));
-          lo.z = __uint_as_float(to_tf32(h[2] - hi.z)); lo.w = __uint_as_float(to_tf32(h[3] - hi.w));
+          lo.x = __uint_as_float(to_tf32(h[4 * kc] - hi.x)); lo.y = __uint_as_float(to_tf32(h[4 * kc + 1] - hi.y));
+          lo.z = __uint_as_float(to_tf32(h[4 * kc + 2] - hi.z)); lo.w = __uint_as_float(to_tf32(h[4 * kc + 3] - hi.w));
           *reinterpret_cast<float4*>(Alo + kc * 32) = lo;
         }
       }
-      // ---- layer 2 on the tensor core ----
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");          // generic-proxy writes of A -> visible to the MMA
-      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");       // orders the previous tile's tcgen05.ld before this MMA
+      asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");       // orders earlier tcgen05.ld of this accumulator before the MMA
       __syncthreads();
+      // ---- layer 2 on the tensor core: D[ntile & 1] = A W2^T ----
       if (tid == 0) {
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        const u32 a_hi = smem_u32(&S.A[0][0]), a_lo = smem_u32(&S.A[1][0]), b_hi = smem_u32(&S.B[0][0]), b_lo = smem_u32(&S.B[1][0]);
+        const u32 d_addr = tmem_d + (ntile & 1u) * 32u;
+        const u32 a_hi = smem_u32(&S.A[0][0]), a_lo = smem_u32(&S.A[SPLIT ? 1 : 0][0]), b_hi = smem_u32(&S.B[0][0]), b_lo = smem_u32(&S.B[SPLIT ? 1 : 0][0]);
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk) umma_tf32(tmem_d, umma_desc(a_hi + kk * 256), umma_desc(b_hi + kk * 256), kk > 0);
+        for (int kk = 0; kk < 4; ++kk) umma_tf32(d_addr, umma_desc(a_hi + kk * 256), umma_desc(b_hi + kk * 256), kk > 0);
         if (SPLIT) {
 #pragma unroll
-          for (int kk = 0; kk < 4; ++kk) umma_tf32(tmem_d, umma_desc(a_lo + kk * 256), umma_desc(b_hi + kk * 256), 1u);
+          for (int kk = 0; kk < 4; ++kk) umma_tf32(d_addr, umma_desc(a_lo + kk * 256), umma_desc(b_hi + kk * 256), 1u);
 #pragma unroll
-          for (int kk = 0; kk < 4; ++kk) umma_tf32(tmem_d, umma_desc(a_hi + kk * 256), umma_desc(b_lo + kk * 256), 1u);
+          for (int kk = 0; kk < 4; ++kk) umma_tf32(d_addr, umma_desc(a_hi + kk * 256), umma_desc(b_lo + kk * 256), 1u);
         }
         asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar_mma) : "memory");
       }
+      // ---- epilogue of the previous tile (its accumulator was complete at the wait above): overlaps this MMA ----
+      if (pend) epilogue((ntile - 1u) & 1u, p_valid, p_ii, p_jj, p_inv);
+      pend = true; p_valid = valid; p_ii = ii; p_jj = jj; p_inv = inv;
+      ++ntile;
+    }
+    if (pend) {                                                            // drain: the staged sources are about to be replaced
       alive = alive && mbar_wait(bar_mma, phase);
       phase ^= 1u;
-      asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-      u32 dr[32];
-      asm volatile(
-          "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, %17, %18, %19, %20, "
-          "%21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-          : "=r"(dr[0]), "=r"(dr[1]), "=r"(dr[2]), "=r"(dr[3]), "=r"(dr[4]), "=r"(dr[5]), "=r"(dr[6]), "=r"(dr[7]), "=r"(dr[8]), "=r"(dr[9]),
-            "=r"(dr[10]), "=r"(dr[11]), "=r"(dr[12]), "=r"(dr[13]), "=r"(dr[14]), "=r"(dr[15]), "=r"(dr[16]), "=r"(dr[17]), "=r"(dr[18]),
-            "=r"(dr[19]), "=r"(dr[20]), "=r"(dr[21]), "=r"(dr[22]), "=r"(dr[23]), "=r"(dr[24]), "=r"(dr[25]), "=r"(dr[26]), "=r"(dr[27]),
-            "=r"(dr[28]), "=r"(dr[29]), "=r"(dr[30]), "=r"(dr[31])
-          : "r"(tmem_d + ((warp * 32u) << 16))
-          : "memory");
-      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-      // ---- epilogue: + b2, tanh, layer 3, 1/r, apply (S-3) ----
-      float out[9];
-#pragma unroll
-      for (int r = 0; r < 9; ++r) out[r] = S.b3[r];
-#pragma unroll
-      for (int o = 0; o < 32; ++o) {
-        const float pre = __uint_as_float(dr[o]) + S.b2[o];
-        const float t = SPLIT ? tanhf(pre) : tanh_mufu(pre);
-        const float4 wa = *reinterpret_cast<const float4*>(&S.w3t[12 * o]);
-        const float4 wb = *reinterpret_cast<const float4*>(&S.w3t[12 * o + 4]);
-        const float wc = S.w3t[12 * o + 8];
-        out[0] = fmaf(wa.x, t, out[0]); out[1] = fmaf(wa.y, t, out[1]); out[2] = fmaf(wa.z, t, out[2]);
-        out[3] = fmaf(wa.w, t, out[3]); out[4] = fmaf(wb.x, t, out[4]); out[5] = fmaf(wb.y, t, out[5]);
-        out[6] = fmaf(wb.z, t, out[6]); out[7] = fmaf(wb.w, t, out[7]); out[8] = fmaf(wc, t, out[8]);
-      }
-      if (valid && tlo + ii != S.sJ[jj]) {                                   // S-5: the pair i == j is skipped
-        const float f0 = S.sFj[3 * jj], f1 = S.sFj[3 * jj + 1], f2 = S.sFj[3 * jj + 2];
-#pragma unroll
-        for (int al = 0; al < 3; ++al)
-          atomicAdd(&S.sU[3 * ii + al], inv * fmaf(out[3 * al], f0, fmaf(out[3 * al + 1], f1, out[3 * al + 2] * f2)));
-      }
+      epilogue((ntile - 1u) & 1u, p_valid, p_ii, p_jj, p_inv);
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
     b += nb;
   }
@@ -233,7 +254,7 @@ __global__ void __launch_bounds__(NT_T) k_near_tc(const float* __restrict__ gw, 
   if (!alive && tid == 0) atomicExch(err_flag, 1u);
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 32;" ::"r"(tmem_d) : "memory");
+  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 64;" ::"r"(tmem_d) : "memory");
 }
 
 // W2 as the B operand of the contraction: tf32 hi part and tf32 remainder, both in the K-major core-matrix layout of the
@@ -258,7 +279,7 @@ void hh_pack_w2_tc(const float* W2 /* [32][32] row-major [out][in] */, float* ou
 
 int hh_near_apply_tc(hh_ctx* ctx) {
   if (ctx->n_leaves <= 0 || ctx->nH <= 0) return HH_OK;
-  const size_t smem = sizeof(NtSmem) + 1024;
+  const size_t smem = (ctx->p.near_path == 2 ? sizeof(NtSmem<2>) : sizeof(NtSmem<1>)) + 1024;
   cudaStream_t s = ctx->stream;
   HH_CUDA(cudaMemsetAsync(&ctx->d_sc->deg_overflow, 0, sizeof(u32), s));   // doubles as the kernel's error flag
   if (ctx->p.near_path == 2) {

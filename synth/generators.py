@@ -65,6 +65,106 @@ def lattice_cloud(nx, ny, nz, spacing, jitter=0.0, seed=0):
     return X.astype(np.float32)
 
 
+def lattice_drop(radius, phi, centre=(0.0, 0.0, 0.0), jitter=0.2, seed=0, a=1.0):
+    """One suspension drop as the paper builds it (Sec. 4.3.1): a primitive cubic lattice at volume
+    fraction phi (spacing h = a (4 pi / 3 / phi)^(1/3)), the points outside the sphere discarded, every position
+    slightly perturbed (uniform in +-jitter per axis; non-overlapping while h - 2 sqrt(3) jitter > 2a).  The sphere
+    centre sits on a lattice point.  The number of particles follows from the lattice; the paper's drop of radius 175
+    at phi = 10 % has 523,305 (its lattice offset is not stated; this one has 536,393)."""
+    h = a * (4.0 * math.pi / 3.0 / phi) ** (1.0 / 3.0)
+    k = int(math.floor(radius / h)) + 1
+    ax = np.arange(-k, k + 1, dtype=np.float64) * h
+    g = np.stack(np.meshgrid(ax, ax, ax, indexing="ij"), -1).reshape(-1, 3)
+    g = g[(g * g).sum(1) <= radius * radius]
+    if jitter:
+        g = g + (uniform01(seed, 0, g.size).reshape(g.shape) - 0.5) * 2.0 * jitter
+    return (g + np.asarray(centre, np.float64)).astype(np.float32)
+
+
+def two_drops(radius=175.0, phi=0.1, gap=0.2, jitter=0.2, seed=0):
+    """The two sedimenting drops of PAPER.md L342: vertically aligned, no horizontal offset, the trailing drop above the
+    leading one.  The initial separation is not stated in the text; `gap` (in radii) is the clearance between the spheres."""
+    lead = lattice_drop(radius, phi, (0.0, 0.0, 0.0), jitter, seed)
+    trail = lattice_drop(radius, phi, (0.0, 0.0, (2.0 + gap) * radius), jitter, seed + 1)
+    return np.concatenate([lead, trail], 0)
+
+
+def filament_sphere(n_fil=5120, n_beads=21, r_b=3.0, n_free=107520, dmin=2.1, seed=0, a=1.0):
+    """The mixture of PAPER.md L369 (Sec. 4.3.2): n_fil straight filaments of n_beads beads (spacing r_b), randomly
+    oriented and positioned inside the inner sphere R_in = 2^(-1/3) R_out, R_out = 4 * 10^(1/3) (n_beads - 1) r_b, and n_free
+    individual particles in the shell between R_in and R_out; any two beads / particles of different objects at least
+    dmin apart.  Random sequential addition in counter order: a candidate that comes within dmin of an earlier
+    object is dropped.  Filaments come first in the output (n_fil * n_beads rows), then the free particles.
+    "Positioned within the inner sphere" is read as: every bead inside it."""
+    from scipy.spatial import cKDTree
+    R_out = 4.0 * 10.0 ** (1.0 / 3.0) * (n_beads - 1) * r_b
+    R_in = 0.5 ** (1.0 / 3.0) * R_out
+    half = 0.5 * (n_beads - 1) * r_b
+    s = (np.arange(n_beads, dtype=np.float64) - 0.5 * (n_beads - 1)) * r_b
+
+    def sphere_dirs(u):
+        cz = 2.0 * u[:, 0] - 1.0
+        sz = np.sqrt(np.maximum(0.0, 1.0 - cz * cz))
+        ang = 2.0 * np.pi * u[:, 1]
+        return np.stack([sz * np.cos(ang), sz * np.sin(ang), cz], 1)
+
+    def add_batch(have, cand):
+        """cand [n_obj][n_pts][3] in counter order: drop objects within dmin of `have` [*][3] or of an EARLIER kept candidate"""
+        n_obj, n_pts = cand.shape[:2]
+        keep = np.ones(n_obj, bool)
+        pts = cand.reshape(-1, 3)
+        if len(have):
+            hit = np.isfinite(cKDTree(have).query(pts, k=1, distance_upper_bound=dmin)[0])
+            keep &= ~hit.reshape(n_obj, n_pts).any(1)
+        pairs = cKDTree(pts).query_pairs(dmin, output_type="ndarray")
+        if len(pairs):
+            oi, oj = pairs[:, 0] // n_pts, pairs[:, 1] // n_pts
+            sel = oi != oj
+            lo, hi = np.minimum(oi[sel], oj[sel]), np.maximum(oi[sel], oj[sel])
+            order = np.lexsort((hi, lo))
+            for i, j in zip(lo[order], hi[order]):
+                if keep[i]:
+                    keep[j] = False                                  # the later object of a close pair goes
+        return cand[keep]
+
+    # filaments: centre uniform in the ball (rejection from the cube), kept if both end beads are inside the inner sphere
+    fil = np.zeros((0, n_beads, 3))
+    start = 0
+    while len(fil) < n_fil:
+        m = int((n_fil - len(fil)) * 3.0) + 64
+        c = (uniform01(seed, 0, 3 * m, start=3 * start).reshape(m, 3) * 2.0 - 1.0) * R_in
+        d = sphere_dirs(uniform01(seed, 4, 2 * m, start=2 * start).reshape(m, 2))
+        start += m
+        ends_ok = (np.linalg.norm(c + half * d, axis=1) <= R_in - a) & (np.linalg.norm(c - half * d, axis=1) <= R_in - a)
+        cand = (c[:, None, :] + s[None, :, None] * d[:, None, :])[ends_ok]
+        fil = np.concatenate([fil, add_batch(fil.reshape(-1, 3), cand)], 0)[:n_fil]
+    beads = fil.reshape(-1, 3)
+    # free particles in the shell, against the filaments and against each other
+    free = np.zeros((0, 3))
+    start = 0
+    while len(free) < n_free:
+        m = int((n_free - len(free)) * 2.6) + 256
+        c = (uniform01(seed, 6, 3 * m, start=3 * start).reshape(m, 3) * 2.0 - 1.0) * R_out
+        start += m
+        r = np.linalg.norm(c, axis=1)
+        c = c[(r >= R_in + a) & (r <= R_out - a)]
+        if len(c):
+            free = np.concatenate([free, add_batch(np.concatenate([beads, free], 0), c[:, None, :])[:, 0, :]], 0)[:n_free]
+    return np.concatenate([beads, free], 0).astype(np.float32), dict(R_out=R_out, R_in=R_in, L_f=(n_beads - 1) * r_b + 2 * a)
+
+
+def mixture_forces(X, n_fil, n_beads, bond=3.0, k=20.0, kappa=50.0, xp=np):
+    """Forces of the filament mixture: harmonic tension k_t = 20 with rest length r_b, COS bending
+    k_b = 50 on the filament beads (the first n_fil * n_beads rows), gravity (0,0,-1) on every particle."""
+    nf = n_fil * n_beads
+    F = xp.zeros_like(X)
+    F[:, 2] -= 1.0
+    Ff = filament_forces(X[:nf], n_fil, n_beads, bond=bond, k=k, kappa=kappa, xp=xp)
+    Ff[:, 2] += 1.0                                                  # filament_forces adds gravity itself
+    F[:nf] += Ff
+    return F
+
+
 def line_points(n):
     """x_i = (i + 1/2)/n on the x axis: the 1-D example of Fig. 4."""
     X = np.zeros((n, 3), dtype=np.float64)
@@ -128,6 +228,8 @@ def xavier_mlp(dims, seed, bias_scale=0.0):
 
 
 # ------------------------------------------------------------------------------- configs
+# kappa_max: 0 = Alg. 2 as printed (the default of the library and of the oracle); c5 opts in to S-18b.
+# near_path: 2 = near-field entries on the tcgen05 tensor cores with split tf32 operands (fp32-class accuracy).
 CONFIGS = {
     # name: BASELINE.json config it realises
     "c1": dict(n=2048, shape="cube", phi=0.1, forces="gaussian", leaf=64, eta=1.0, tol=1e-4,
@@ -140,6 +242,11 @@ CONFIGS = {
                rcut3=4.0, steps=1, dt=0.0),
     "c5": dict(n=1000000, shape="chains", phi=0.1, forces="filament", leaf=64, eta=1.0, tol=1e-4,
                rcut3=4.0, steps=100, dt=0.005, n_chains=20000, n_beads=50, kappa_max=50.0),   # S-18b: chains need 50 for the 1e-5 bar
+    # the paper's own workloads at the paper's parameters; random-init MLPs
+    "p1": dict(n=None, shape="two_drops", phi=0.1, forces="gravity", leaf=50, eta=1.0, tol=0.1, rcut3=4.0, steps=50, dt=0.01,
+               radius=175.0),
+    "p2": dict(n=215040, shape="filament_sphere", phi=None, forces="mixture", leaf=50, eta=1.0, tol=0.02, rcut3=4.0, steps=1,
+               dt=0.002, n_chains=5120, n_beads=21, n_free=107520),
 }
 
 
@@ -147,6 +254,18 @@ def config(name, n=None):
     """(cfg dict, X, F) for a named config; `n` overrides the particle count while keeping
     the volume fraction (used for bounded CPU samples of the same workload)."""
     cfg = dict(CONFIGS[name])
+    if cfg["shape"] == "two_drops":
+        scale = 1.0 if n is None else (n / 1072786.0) ** (1.0 / 3.0)      # n shrinks the radius at the same volume fraction
+        X = two_drops(cfg["radius"] * scale, cfg["phi"])
+        cfg["n"] = len(X)
+        return cfg, X, gravity_forces(len(X))
+    if cfg["shape"] == "filament_sphere":
+        f = 1.0 if n is None else n / cfg["n"]
+        cfg["n_chains"], cfg["n_free"] = max(1, int(cfg["n_chains"] * f)), max(1, int(cfg["n_free"] * f))
+        X, _ = filament_sphere(cfg["n_chains"], cfg["n_beads"], 3.0, cfg["n_free"])
+        cfg["n"] = len(X)
+        F = mixture_forces(X.astype(np.float64), cfg["n_chains"], cfg["n_beads"]).astype(np.float32)
+        return cfg, X, F
     if n is not None:
         if cfg["shape"] == "chains":
             cfg["n_chains"] = max(1, n // cfg["n_beads"])

@@ -115,3 +115,46 @@ def test_configs_match_baseline_json():
     assert "20,000 chains of 50 beads" in txt and synth.CONFIGS["c5"]["n_chains"] == 20000
     cfg, X, F = synth.config("c2", n=512)
     assert X.shape == (512, 3) and np.all(F == [0, 0, -1])
+
+
+def test_two_drops_as_the_paper_builds_them():
+    """lattice at phi = 10 %, points outside the sphere discarded, slightly perturbed; two drops vertically
+    aligned.  At a reduced radius (the generator is the same at 175)."""
+    R, phi = 40.0, 0.1
+    X = synth.two_drops(R, phi).astype(np.float64)
+    n1 = len(synth.lattice_drop(R, phi))
+    assert len(X) == 2 * n1
+    assert abs(n1 / (phi * R ** 3) - 1.0) < 0.03                     # N = phi R^3 / a^3 up to lattice discreteness
+    lead, trail = X[:n1], X[n1:]
+    assert np.abs(lead.mean(0)).max() < 0.2 and np.abs(trail.mean(0)[:2]).max() < 0.2      # no horizontal offset
+    assert abs(trail.mean(0)[2] - 2.2 * R) < 0.2
+    assert np.linalg.norm(lead, axis=1).max() <= R + 0.2 * math.sqrt(3) + 1e-4
+    from scipy.spatial import cKDTree
+    d, _ = cKDTree(X).query(X, k=2)
+    h = (4 * math.pi / 3 / phi) ** (1 / 3)
+    assert d[:, 1].min() >= h - 2 * 0.2 * math.sqrt(3) - 1e-4 > 2.0     # non-overlapping
+    assert np.array_equal(synth.two_drops(R, phi), synth.two_drops(R, phi))
+
+
+def test_filament_sphere_of_the_paper():
+    """R_out = 4 * 10^(1/3) (N_b - 1) r_b, R_in = 2^(-1/3) R_out, filaments inside R_in, particles in the
+    shell, minimum distance 2.1 between objects; equal numbers of filament beads and free particles."""
+    nf, nb, nfree = 256, 21, 5376
+    X, info = synth.filament_sphere(nf, nb, 3.0, nfree)
+    X = X.astype(np.float64)
+    assert len(X) == nf * nb + nfree and nf * nb == nfree
+    assert abs(info["R_out"] - 4 * 10 ** (1 / 3) * 60) < 1e-9 and abs(info["R_in"] - info["R_out"] / 2 ** (1 / 3)) < 1e-9 and info["L_f"] == 62
+    r = np.linalg.norm(X, axis=1)
+    assert r[:nf * nb].max() <= info["R_in"] and r[nf * nb:].min() >= info["R_in"] and r.max() <= info["R_out"]
+    P = X[:nf * nb].reshape(nf, nb, 3)
+    assert np.allclose(np.linalg.norm(P[:, 1:] - P[:, :-1], axis=-1), 3.0, atol=1e-4)
+    from scipy.spatial import cKDTree
+    pairs = cKDTree(X).query_pairs(2.1 - 1e-4, output_type="ndarray")
+    assert len(pairs) == 0
+    F = synth.mixture_forces(X, nf, nb)
+    assert np.allclose(F[nf * nb:], [0, 0, -1]) and np.abs(F[:nf * nb] - [0, 0, -1]).max() < 0.01    # straight, at rest length
+    # a bent, stretched filament feels restoring forces that sum to zero (internal forces)
+    Y = X.copy()
+    Y[:nb] += np.random.default_rng(0).normal(0, 0.2, (nb, 3))
+    G = synth.mixture_forces(Y, nf, nb)
+    assert np.abs((G[:nb] - [0, 0, -1]).sum(0)).max() < 1e-9 and np.abs(G[:nb] - [0, 0, -1]).max() > 0.1

@@ -30,6 +30,9 @@ if ROOT not in sys.path:
 METRIC = "H-matvec particles/s (whole step: tree + blocks + ACA + near + far + three-body)"
 UNIT = "particles/s"
 FAR_BYTES_PER_UNIT = 36          # bytes of fp32 factors read per (row or column) x block-rank (DESIGN.md far-field)
+# dram__bytes_read.sum + dram__bytes_write.sum of the k_far launches / their algorithmic factor bytes, from the ncu --set full
+# capture summarised in profiles/r02_far_traffic_c3.md (per launch; the bench line scales it to the launches of one step)
+FAR_TRAFFIC_RATIO = None
 ORACLE_SAMPLE_N = {"c1": 2048, "c2": 8192, "c3": 24576, "c4": 16384, "c5": 16000, "p1": 60000, "p2": 60000}
 
 
@@ -310,7 +313,8 @@ def run_gpu(args):
                                       "sum_rank", "aca_entries", "factor_bytes", "aca_not_converged", "aca_singular", "fallback_entries", "n_faces")},
         "roofline": {"kernel": "k_far (far-field apply U^tau += C (Q F^sigma), all size classes and arena batches of one step)",
                      "bound": "hbm", "achieved": far_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": far_gbs / hbm_peak,
-                     "traffic": None, "traffic_note": "not collected in this run (needs ncu); measured dram__bytes_read = 1.02 x algorithmic bytes, profiles/r01b_far_traffic.md",
+                     "traffic": FAR_TRAFFIC_RATIO * far_bytes if FAR_TRAFFIC_RATIO else None,
+                     "traffic_note": "dram bytes of the k_far launches of one step = ncu-measured ratio x algorithmic bytes (profiles/r02_far_traffic_c3.md); not re-collected in this run",
                      "peak_source": peak_src, "share_of_step": far_ms / step_ms,
                      "algorithmic_bytes_per_step": far_bytes, "ms_per_step": far_ms},
         "wall_s_timed_region": t_wall,
@@ -320,10 +324,60 @@ def run_gpu(args):
         t, n, cores = oracle_step_sample(args.workload, n_s)
         line["cpu_baseline"] = {"value": n / t, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": "one full oracle step (fp64) on a %d-particle cloud of the same recipe, %.1f s" % (n, t)}
-    print(json.dumps(line), flush=True)
     ctx.close()
+    if args.with_c4 and world == 1 and args.workload == "c3":
+        # the metric is quoted at 1M AND 10M particles: the 10M point (BASELINE.json configs[3]) rides along as a sub-record
+        del ctx, Xd, Fd, Ud, flush
+        torch.cuda.empty_cache()
+        line["c4"] = sub_record("c4", args, dev, hbm_peak)
+    print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
+
+
+def sub_record(workload, args, dev, hbm_peak):
+    """one warm-up + one timed hh_step of `workload` on this GPU (the 10M half of the metric beside the 1M line): its own
+    ms_per_step, stages, counts and far-field roofline.  Inputs resident in HBM, L2 flushed, CUDA events."""
+    import torch
+    import synth
+    import paper_2505_08174_b200 as hh
+    cfg, X, F = make_inputs(workload, 0)
+    N = len(X)
+    mlp2 = synth.xavier_mlp(synth.MLP2_DIMS, 1)
+    mlp3 = synth.xavier_mlp(synth.MLP3_DIMS, 3) if cfg["rcut3"] > 0 else None
+    free, _ = torch.cuda.mem_get_info(dev)
+    ws = int(min(free * 0.85, args.workspace_gb * (1 << 30)))
+    ctx = hh.Context(mlp2, mlp3, leaf_size=cfg["leaf"], eta=cfg["eta"], aca_tol=cfg["tol"], rcut3=cfg["rcut3"],
+                     kappa_max=float(cfg.get("kappa_max", 0.0)), near_path=args.near_path, aca_precision=args.aca_precision,
+                     workspace_bytes=ws, device=dev)
+    ctx.enable_timing(True)
+    stream = torch.cuda.current_stream(dev)
+    Xd, Fd = torch.from_numpy(X).to(dev), torch.from_numpy(F).to(dev)
+    Ud = torch.empty_like(Fd)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ms = None
+    for _ in range(2):                                                  # warm-up, then the timed step
+        flush.fill_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        ctx.step(Xd, Fd, Ud, dt=float(cfg["dt"]))
+        e1.record(stream)
+        e1.synchronize()
+        ms = e0.elapsed_time(e1)
+    st = ctx.stats()
+    assert torch.isfinite(Ud).all().item(), "non-finite velocities"
+    far_gbs = st["factor_bytes"] / (st["ms_far"] * 1e-3) / 1e9 if st["ms_far"] > 0 else 0.0
+    out = {"workload": workload_name(workload, cfg), "steps": 1, "warmup": 1, "ms_per_step": ms, "value": N / (ms * 1e-3), "unit": UNIT,
+           "stages_ms": {k: st[k] for k in ("ms_tree", "ms_blocks", "ms_aca", "ms_near", "ms_far", "ms_three", "ms_other")},
+           "counts": {k: st[k] for k in ("n_admissible", "n_inadmissible", "near_entries", "sum_rank", "aca_entries", "factor_bytes", "aca_batches",
+                                         "aca_not_converged", "aca_singular")},
+           "gpu_launches": int(st["n_launches"]),
+           "roofline": {"kernel": "k_far", "bound": "hbm", "achieved": far_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": far_gbs / hbm_peak,
+                        "algorithmic_bytes_per_step": float(st["factor_bytes"]), "ms_per_step": st["ms_far"]}}
+    ctx.close()
+    del ctx, Xd, Fd, Ud, flush
+    torch.cuda.empty_cache()
+    return out
 
 
 def main():
@@ -342,6 +396,7 @@ def main():
     ap.add_argument("--near-path", type=int, default=2, choices=[0, 1, 2], help="0 fp32 ALU, 1 tcgen05 tf32 + tanh.approx (2e-3), 2 tcgen05 split tf32 + tanhf")
     ap.add_argument("--aca-precision", type=int, default=0, choices=[0, 1], help="1 = fp64 entries and residuals in Alg. 2 (parity mode)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    ap.add_argument("--no-c4", dest="with_c4", action="store_false", help="skip the 10M-particle sub-record of the default (c3) run")
     args = ap.parse_args()
     args.warmup_ref = min(args.warmup, 1)
     if args.impl == "reference":

@@ -15,7 +15,7 @@ LIB = os.path.join(HERE, "libhh.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--use_fast_math=false",
          "-Xcompiler", "-fPIC,-O2,-Wall", "-Xptxas", "-v", "--fmad=true"]
-FLAGS = [f for f in FLAGS if f != "--use_fast_math=false"] + os.environ.get("HH_NVCC_EXTRA", "").split()   # e.g. -DHH_FAST_TANH
+FLAGS = [f for f in FLAGS if f != "--use_fast_math=false"] + os.environ.get("HH_NVCC_EXTRA", "").split()
 
 
 def _deps_mtime():

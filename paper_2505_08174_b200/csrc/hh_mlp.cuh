@@ -4,31 +4,9 @@
 #pragma once
 #include "hh_internal.cuh"
 
-// S-6: the fp32 path needs a tanh good to a few ulp.  Default: CUDA's tanhf (<= 2 ulp, ~25 instructions, half of the
-// instructions of an entry).  -DHH_FAST_TANH selects a branch-free form of the same accuracy class (odd-symmetric:
-// |x| < 0.55: x + x^3 P(x^2), degree-4 P fitted to (tanh x - x)/x^3, 1.1 ulp; else 1 - 2/(2^(2|x| log2 e) + 1) with
-// MUFU ex2 / rcp, no cancellation since tanh >= 0.5 there; saturates to 1 through inf).  Not the default until the
-// zeta = 1e-5 parity case has been run often enough with it ("tried").
-__device__ __forceinline__ float hh_tanh_fast(float x) {
-  const float t = fabsf(x), u = t * t;
-  float p = fmaf(-0.006274234503507614f, u, 0.021071674302220345f);
-  p = fmaf(p, u, -0.05385230854153633f);
-  p = fmaf(p, u, 0.13332585990428925f);
-  p = fmaf(p, u, -0.33333316445350647f);
-  const float ys = fmaf(p, t * u, t);
-  float e, r;
-  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(t * 2.8853900817779268f));
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e + 1.0f));
-  const float yl = fmaf(r, -2.0f, 1.0f);
-  return copysignf(t < 0.55f ? ys : yl, x);
-}
-#ifndef HH_TANH
-#ifdef HH_FAST_TANH
-#define HH_TANH(x) hh_tanh_fast(x)
-#else
+// S-6: the fp32 path needs a tanh good to a few ulp: CUDA's tanhf (<= 2 ulp).  tanh.approx (2^-11) is used only on the 2e-3
+// tensor-core path (hh_near_tc.cu, near_path = 1).
 #define HH_TANH(x) tanhf(x)
-#endif
-#endif
 
 // Packed layout (floats): W1 [H][INP] | b1 [H] | W2 [H][H] | b2 [H] | W3T [H][12] | b3 [12]
 template <int INP, int H>

@@ -206,7 +206,7 @@ def run_gpu(args):
         if val is not None:
             cfg[key] = val                                              # sweeps of config 3 (eta, zeta); otherwise the config's own
     N = len(X)
-    mlp2 = synth.xavier_mlp(synth.MLP2_DIMS, 1)
+    mlp2 = synth.xavier_mlp(synth.MLP2_PAPER_DIMS if args.paper_mlp else synth.MLP2_DIMS, 1)
     mlp3 = synth.xavier_mlp(synth.MLP3_DIMS, 3) if cfg["rcut3"] > 0 else None
     free, _ = torch.cuda.mem_get_info(dev)
     ws = int(min(free * 0.85, args.workspace_gb * (1 << 30)))
@@ -301,6 +301,7 @@ def run_gpu(args):
                    "l2": "explicit 256 MB flush write between timed iterations; each step also streams its factor arena (>> L2)",
                    "arena_gb": st["arena_bytes"] / 2 ** 30, "aca_batches_per_step": st["aca_batches"],
                    "near_path": "%d (%s)" % (args.near_path, ["fp32 ALU", "tcgen05 tf32 + tanh.approx (2e-3 path)", "tcgen05 split tf32 + tanhf (fp32-class)"][args.near_path]),
+                   "mlp2": "4-128-512-128-9 (paper-size hidden layers, tcgen05 tf32 tile, tolerance 2e-3)" if args.paper_mlp else "4-32-32-9",
                    "aca_precision": "%d (%s)" % (args.aca_precision, ["fp32 entries in Alg. 2", "fp64 entries and residuals in Alg. 2 (parity mode)"][args.aca_precision])},
         "clocks": clk,
         "e2e": {"value": world * N * ke / e2e_s, "unit": UNIT, "h2d_bytes_per_step": 24 * N, "d2h_bytes_per_step": 24 * N,
@@ -395,6 +396,7 @@ def main():
     ap.add_argument("--kappa-max", type=float, default=None, help="S-18b limit on the pivot-block condition number")
     ap.add_argument("--near-path", type=int, default=2, choices=[0, 1, 2], help="0 fp32 ALU, 1 tcgen05 tf32 + tanh.approx (2e-3), 2 tcgen05 split tf32 + tanhf")
     ap.add_argument("--aca-precision", type=int, default=0, choices=[0, 1], help="1 = fp64 entries and residuals in Alg. 2 (parity mode)")
+    ap.add_argument("--paper-mlp", action="store_true", help="two-body MLP with the paper's hidden layers 128/512/128 (tensor-core tile)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     ap.add_argument("--no-c4", dest="with_c4", action="store_false", help="skip the 10M-particle sub-record of the default (c3) run")
     args = ap.parse_args()

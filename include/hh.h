@@ -49,7 +49,9 @@ typedef struct hh_ctx hh_ctx;           /* opaque, owned by the library */
 
 /* An MLP  y = W_L tanh( ... tanh(W_1 x + b_1) ... ) + b_L  (tanh on hidden layers only; PAPER.md L92,
  * S-4).  Supported shapes: two-body 4->32->32->9 (features [r_hat(3), a/r], Eq. (4) L85 + config),
- * three-body 7->64->64->9 (features [X_j-X_i, X_k-X_i, |X_j-X_k|]).
+ * three-body 7->64->64->9 (features [X_j-X_i, X_k-X_i, |X_j-X_k|]); and, for the two-body term, the paper-size network
+ * 4->128->512->128->9 (n_layers = 4; L92), evaluated on the tcgen05 tensor cores with tf32 operands and tanh.approx
+ * (tolerance 2e-3; meant for the paper's own ACA tolerances zeta >= 1e-2; lock-step ACA only, no S-18b, no parity mode).
  *   dims : HOST   int32[n_layers+1]
  *   W, b : HOST   arrays of n_layers DEVICE pointers; W[l] is [dims[l+1]][dims[l]] row-major fp32,
  *                 b[l] is [dims[l+1]] fp32.  Copied into the context at hh_create. */

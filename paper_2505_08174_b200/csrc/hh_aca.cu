@@ -487,6 +487,7 @@ int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next) {
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   const DevScalars& h = *ctx->h_sc;
+  if (ctx->mlp2_wide && h.deg_overflow) return hh_fail(ctx, HH_ERR_CUDA, "paper-size MLP entries (ACA): an mbarrier wait timed out");
   ctx->res_first = first;
   ctx->res_next = nx;
   *next = nx;

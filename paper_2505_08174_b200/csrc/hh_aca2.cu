@@ -20,6 +20,7 @@
 //                     next column; arena space for the next HH_RC ranks
 // Storage, arena chunks, table rows and the pivot record are those of hh_aca.cu (the far-field kernel reads both).
 #include "hh_mlp.cuh"
+#include "hh_wide.cuh"
 
 #define GR 16                    /* entries per granule = half a warp                                   */
 #define A2_T 256                 /* threads of the entry-evaluating kernels                              */
@@ -210,11 +211,14 @@ __device__ __forceinline__ void a2_norm_granule(const A2Args& A, u32 gi, u32 cou
 // Measured and dropped: prefetching those lines into L2 before the MLP arithmetic (+5 %), staging them
 // through shared memory with cp.async (+29 %), one loop over both slots (+22 %, spills).
 // F64 (aca_precision = 1, parity mode): the entry and the residual subtraction in fp64, rounded once when stored.
-template <bool COLS, bool F64>
+// PRE (paper-size MLP, hh_wide.cuh): the raw entries were written into the rank-k slot by k2_eval_wide; they are loaded here.
+template <bool COLS, bool F64, bool PRE = false>
 __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncount) {
-  __shared__ __align__(16) float sw[F64 ? 2 * HH_MLP2_FLOATS : HH_MLP2_FLOATS];
-  if (F64) load_weights(sw, reinterpret_cast<const float*>(A.w2d), 2 * HH_MLP2_FLOATS);
-  else load_weights(sw, A.w2, HH_MLP2_FLOATS);
+  __shared__ __align__(16) float sw[PRE ? 4 : (F64 ? 2 * HH_MLP2_FLOATS : HH_MLP2_FLOATS)];
+  if (!PRE) {
+    if (F64) load_weights(sw, reinterpret_cast<const float*>(A.w2d), 2 * HH_MLP2_FLOATS);
+    else load_weights(sw, A.w2, HH_MLP2_FLOATS);
+  }
   __syncthreads();
   const u32 lane = threadIdx.x & 31, half = lane >> 4, l16 = lane & 15, warp = threadIdx.x >> 5;
   const uint2* gl = COLS ? A.gn : A.gm;
@@ -229,7 +233,22 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
     // (b) the entries
     float v[2][9];
     double vd[F64 ? 2 : 1][9];
-    {
+    if (PRE) {
+#pragma unroll
+      for (int e = 0; e < 2; ++e) {
+        const u32 gi = 4 * tile + 2 * e + half;
+        const bool gv = gi < count;
+        const uint2 g = gl[gv ? gi : count - 1];
+        const BlkState& s = A.st[g.x];
+        const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
+        const u32 len = COLS ? s.n : s.m, lenp = COLS ? np : mp, idx = g.y + l16;
+        const bool ok = gv && s.status == 0 && idx < len;
+        const float* src = chunk_ptr(A, A.tab + (size_t)g.x * HH_TAB_STRIDE, s.k) +
+                           (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(s.k % HH_RC) * 9 * np : (size_t)(s.k % HH_RC) * 9 * mp);
+#pragma unroll
+        for (int r = 0; r < 9; ++r) v[e][r] = ok ? src[(size_t)r * lenp + idx] : 0.f;
+      }
+    } else {
       float xi[2][3], xj[2][3];
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
@@ -380,6 +399,49 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
     }
 }
 
+// ---- paper-size MLP: the entries of lines 4 / 7 for all active blocks, 128 per tensor-core tile (8 granules), stored raw
+// in the slot of rank k (gather coordinates -> network inference -> scatter into C / Q) ----
+template <bool COLS>
+__global__ void __launch_bounds__(128) k2_eval_wide(A2Args A, const float* __restrict__ gw, u32 count, u32* __restrict__ err_flag) {
+  extern __shared__ __align__(1024) unsigned char we_raw[];
+  WideSmem& S = *reinterpret_cast<WideSmem*>(we_raw);
+  wide_setup(S, gw);
+  const u32 tid = threadIdx.x, l16 = tid & 15;
+  const uint2* gl = COLS ? A.gn : A.gm;
+  const u32 ntiles = (count + 7) / 8;
+  bool alive = true;
+  for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const u32 gi = 8 * tile + (tid >> 4);
+    const bool gv = gi < count;
+    const uint2 g = gl[gv ? gi : count - 1];
+    const BlkState& s = A.st[g.x];
+    const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
+    const u32 len = COLS ? s.n : s.m, lenp = COLS ? np : mp, idx = g.y + l16;
+    const u32 ic = idx < len ? idx : len - 1;
+    const u32 ti = COLS ? s.tlo + (u32)(s.ik < 0 ? 0 : s.ik) : s.tlo + ic;
+    const u32 sj = COLS ? s.slo + ic : s.slo + (u32)s.jk;
+    float xi[3], xj[3], x[4], inv, out[9];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { xi[d] = A.Xs[3 * (size_t)ti + d]; xj[d] = A.Xs[3 * (size_t)sj + d]; }
+    {
+      const float rx = xj[0] - xi[0], ry = xj[1] - xi[1], rz = xj[2] - xi[2];
+      float d = sqrtf(fmaf(rx, rx, fmaf(ry, ry, rz * rz)));
+      d = fmaxf(d, 1e-12f * A.a);
+      inv = 1.0f / d;
+      x[0] = rx * inv; x[1] = ry * inv; x[2] = rz * inv; x[3] = A.a * inv;
+    }
+    alive = wide_tile(S, gw, x, out) && alive;
+    if (gv && s.status == 0 && idx < len) {
+      float* dst = chunk_ptr(A, A.tab + (size_t)g.x * HH_TAB_STRIDE, s.k) +
+                   (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(s.k % HH_RC) * 9 * np : (size_t)(s.k % HH_RC) * 9 * mp);
+#pragma unroll
+      for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp + idx] = out[r] * inv;
+    }
+  }
+  if (!alive && tid == 0) atomicExch(err_flag, 1u);
+  wide_teardown(S);
+}
+
 __device__ __forceinline__ void a2_decode(unsigned long long key, float& score, int& idx) {
   score = key ? __uint_as_float((u32)(key >> 32)) : -1.f;
   idx = key ? (int)(0xffffffffu - (u32)key) : -1;
@@ -510,6 +572,12 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   const u32 per_block_units = (u32)((per_block_bytes + 127) / 128);
   const u64 total_units = ctx->scratch_bytes / 128;
   u32 end_cap = nG;
+  const size_t wsm = sizeof(WideSmem) + 1024;
+  if (ctx->mlp2_wide) {
+    HH_CUDA(cudaFuncSetAttribute(k2_eval_wide<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsm));
+    HH_CUDA(cudaFuncSetAttribute(k2_eval_wide<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)wsm));
+    HH_CUDA(cudaMemsetAsync(&ctx->d_sc->deg_overflow, 0, sizeof(u32), s));   // doubles as the tensor-core kernels' error flag
+  }
   for (int attempt = 0; attempt < 24; ++attempt) {
     k2_batch_range<<<HH_N + 1, 1, 0, s>>>(ctx->unit_prefix, (u32)first, end_cap, total_units > 64 ? total_units - 64 : 0, chunks_pred,
                                           per_block_units, ctx->d_sc);
@@ -561,11 +629,20 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       const unsigned cap = (unsigned)ctx->n_sm * 2 * 4;
       unsigned g1 = cdiv(cdiv(gmc, 4), A2_T / 32), g2 = cdiv(cdiv(gnc, 4), A2_T / 32);
       const unsigned gr = (g1 < cap ? g1 : cap), gc = (g1 > g2 ? g1 : g2) < cap ? (g1 > g2 ? g1 : g2) : cap;
+      if (ctx->mlp2_wide) {
+        const unsigned t1 = cdiv(gmc, 8), t2 = cdiv(gnc, 8), nsm = (unsigned)ctx->n_sm;
+        k2_eval_wide<false><<<HH_N + (t1 < nsm ? t1 : nsm), 128, wsm, s>>>(A, ctx->w2w, gmc, &ctx->d_sc->deg_overflow);
+        k2_step<false, false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
+        k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
+        k2_eval_wide<true><<<HH_N + (t2 < nsm ? t2 : nsm), 128, wsm, s>>>(A, ctx->w2w, gnc, &ctx->d_sc->deg_overflow);
+        k2_step<true, false, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
+      } else {
       if (ctx->p.aca_precision) k2_step<false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
       else k2_step<false, false><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
       k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
       if (ctx->p.aca_precision) k2_step<true, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);   // + line 6 (normalisation)
       else k2_step<true, false><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
+      }
       k2_fin<<<HH_N + gb, 256, 0, s>>>(A);
       HH_LAUNCH_CHECK();
     }

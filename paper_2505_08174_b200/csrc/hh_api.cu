@@ -35,6 +35,7 @@ static int carve(hh_ctx* ctx, int64_t N) {
   ctx->w3 = c.take<float>(HH_MLP3_FLOATS);
   ctx->w2d = c.take<double>(HH_MLP2_FLOATS);
   ctx->w2tc = c.take<float>(2 * 1024);
+  ctx->w2w = c.take<float>(hh_wide_floats());
   for (int k = 0; k < 2; ++k) { ctx->keys[k] = c.take<u64>(N); ctx->idx[k] = c.take<u32>(N); }
   ctx->hist_cap = (size_t)((ctx->cap_pairs > N ? ctx->cap_pairs : N) / 8 + 8192);
   ctx->hist = c.take<u32>(ctx->hist_cap);
@@ -174,8 +175,18 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   HH_CUDA(cudaMemsetAsync(ctx->d_sc, 0, sizeof(DevScalars), ctx->stream));
   for (int k = 0; k < 8; ++k) HH_CUDA(cudaEventCreate(&ctx->ev[k]));
   std::vector<float> pk;
+  if (mlp2->n_layers == 4) {                        // the paper-size network: tensor-core tile of hh_wide.cuh
+    if (params->kappa_max > 0.f || params->aca_precision != 0)
+      return hh_fail(ctx, HH_ERR_UNSUPPORTED, "the paper-size MLP path has neither the S-18b dense fallback nor the fp64 parity mode");
+    std::vector<float> pw(hh_wide_floats());
+    r = hh_pack_wide(ctx, mlp2, pw.data());
+    if (r != HH_OK) return hh_fail(ctx, r, "a 4-layer two-body MLP must be 4->128->512->128->9 with device weight pointers");
+    HH_CUDA(cudaMemcpyAsync(ctx->w2w, pw.data(), pw.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    HH_CUDA(cudaStreamSynchronize(ctx->stream));
+    ctx->mlp2_wide = 1;
+  } else {
   r = pack_mlp(ctx, mlp2, 4, HH_MLP2_INP, HH_MLP2_H, pk);
-  if (r != HH_OK) return hh_fail(ctx, r, "two-body MLP must be 4->32->32->9 with device weight pointers");
+  if (r != HH_OK) return hh_fail(ctx, r, "two-body MLP must be 4->32->32->9 (or 4->128->512->128->9) with device weight pointers");
   HH_CUDA(cudaMemcpyAsync(ctx->w2, pk.data(), pk.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
   std::vector<double> pkd(pk.begin(), pk.end());
   std::vector<float> w2tc(2 * 1024);
@@ -183,6 +194,7 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   HH_CUDA(cudaMemcpyAsync(ctx->w2tc, w2tc.data(), w2tc.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
   HH_CUDA(cudaMemcpyAsync(ctx->w2d, pkd.data(), pkd.size() * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
   HH_CUDA(cudaStreamSynchronize(ctx->stream));
+  }
   if (mlp3) {
     r = pack_mlp(ctx, mlp3, 7, HH_MLP3_INP, HH_MLP3_H, pk);
     if (r != HH_OK) return hh_fail(ctx, r, "three-body MLP must be 7->64->64->9 with device weight pointers");
@@ -206,6 +218,8 @@ extern "C" int hh_set_params(hh_ctx* ctx, const hh_params* params) {
   if (!ctx) return HH_ERR_INVALID_ARG;
   if (!check_params(params)) return hh_fail(ctx, HH_ERR_INVALID_ARG, "invalid parameters");
   if (params->rcut3 > 0.f && !ctx->have_mlp3) return hh_fail(ctx, HH_ERR_INVALID_ARG, "rcut3 > 0 needs a three-body MLP");
+  if (ctx->mlp2_wide && (params->kappa_max > 0.f || params->aca_precision != 0))
+    return hh_fail(ctx, HH_ERR_UNSUPPORTED, "the paper-size MLP path has neither the S-18b dense fallback nor the fp64 parity mode");
   if (params->leaf_size != ctx->p.leaf_size) ctx->tree_ok = ctx->blocks_ok = 0;
   if (params->eta != ctx->p.eta) ctx->blocks_ok = 0;
   ctx->res_first = ctx->res_next = 0;               // factors depend on tol / rank cap / rule / kappa_max
@@ -225,6 +239,7 @@ extern "C" int hh_set_pair_capacity(hh_ctx* ctx, int64_t pairs_per_particle) {
 // 0 = lock-step over the batch (default), 1 = one CTA per admissible block (the first form; kept for comparison)
 extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
   if (!ctx || (impl != 0 && impl != 1)) return HH_ERR_INVALID_ARG;
+  if (impl == 1 && ctx->mlp2_wide) return hh_fail(ctx, HH_ERR_UNSUPPORTED, "the paper-size MLP runs in the lock-step form only");
   ctx->aca_impl = impl;
   ctx->res_first = ctx->res_next = 0;
   return HH_OK;
@@ -480,5 +495,5 @@ extern "C" int hh_eval_entries(hh_ctx* ctx, const float* Xi, const float* Xj, in
   if (!ctx) return HH_ERR_INVALID_ARG;
   if (!Xi || !Xj || !M || n < 0) return hh_fail(ctx, HH_ERR_INVALID_ARG, "hh_eval_entries: null pointer");
   if (n == 0) return HH_OK;
-  return hh_entries_eval(ctx, Xi, Xj, n, M);
+  return ctx->mlp2_wide ? hh_entries_eval_wide(ctx, Xi, Xj, n, M) : hh_entries_eval(ctx, Xi, Xj, n, M);
 }

@@ -47,27 +47,6 @@ __global__ void __launch_bounds__(T, 1024 / T) k_far(const uint2* __restrict__ P
       sF[c][j] = j < nt ? Fs[3 * (size_t)(slo + j0) + t] : 0.f;
     }
     __syncthreads();
-    if (JT <= 256) {
-      // small size classes (the whole sigma fits one tile): one work item per (rank, float4 of columns), flattened over
-      // the CTA, so a 44-column block keeps every lane loading (a warp per rank would leave 20 of 32 lanes idle and
-      // serialise the ranks); partial t_k go to shared memory with three atomics per item
-      const u32 q4 = ntp / 4, items = (u32)l * q4;
-      for (u32 it = tid; it < items; it += T) {
-        const u32 k = it / q4, j4 = it - k * q4;
-        const float* Qk = arena + (size_t)sch[k / HH_RC] * HH_UNIT_FLOATS + (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np + j0;
-        float4 q[9];
-#pragma unroll
-        for (int e = 0; e < 9; ++e) q[e] = ldg_stream(reinterpret_cast<const float4*>(Qk + (size_t)e * np) + j4);
-        const float4 fx = *reinterpret_cast<const float4*>(&sF[0][4 * j4]);
-        const float4 fy = *reinterpret_cast<const float4*>(&sF[1][4 * j4]);
-        const float4 fz = *reinterpret_cast<const float4*>(&sF[2][4 * j4]);
-#define DOT4(a, b) ((a).x * (b).x + (a).y * (b).y + (a).z * (b).z + (a).w * (b).w)
-        atomicAdd(&st[3 * k], DOT4(q[0], fx) + DOT4(q[1], fy) + DOT4(q[2], fz));
-        atomicAdd(&st[3 * k + 1], DOT4(q[3], fx) + DOT4(q[4], fy) + DOT4(q[5], fz));
-        atomicAdd(&st[3 * k + 2], DOT4(q[6], fx) + DOT4(q[7], fy) + DOT4(q[8], fz));
-      }
-      continue;
-    }
     const u32 nsub = (ntp + FAR_SUB - 1) / FAR_SUB;
     for (u32 u = warp; u < (u32)l * nsub; u += NW) {
       const u32 k = u / nsub, sb = u - k * nsub;
@@ -81,6 +60,7 @@ __global__ void __launch_bounds__(T, 1024 / T) k_far(const uint2* __restrict__ P
         const float4 fx = *reinterpret_cast<const float4*>(&sF[0][c0 + 4 * j4]);
         const float4 fy = *reinterpret_cast<const float4*>(&sF[1][c0 + 4 * j4]);
         const float4 fz = *reinterpret_cast<const float4*>(&sF[2][c0 + 4 * j4]);
+#define DOT4(a, b) ((a).x * (b).x + (a).y * (b).y + (a).z * (b).z + (a).w * (b).w)
         a0 += DOT4(q[0], fx) + DOT4(q[1], fy) + DOT4(q[2], fz);
         a1 += DOT4(q[3], fx) + DOT4(q[4], fy) + DOT4(q[5], fz);
         a2 += DOT4(q[6], fx) + DOT4(q[7], fy) + DOT4(q[8], fz);
@@ -115,7 +95,9 @@ __global__ void __launch_bounds__(T, 1024 / T) k_far(const uint2* __restrict__ P
 // CTA sizes per size class (max(m,n) > 256, <= 256, <= 128, <= 64) and the 64-register cap (32 warps per SM) are measured,
 // not derived: the kernel is bound by per-CTA start-up latency and load concurrency.  512 threads / 70 registers for the
 // first class gave 4.28 TB/s at c3, 256 threads / 64 registers 5.03 TB/s (c4: 4.52 -> 5.06 TB/s); halving the threads of
-// every class again helps c3's ragged 64-particle leaves slightly but costs 15 % at c4's 128-particle leaves.
+// every class again helps c3's ragged 64-particle leaves slightly but costs 15 % at c4's 128-particle leaves.  Round 2: one work
+// item per (rank, float4 of columns) flattened over the CTA for the classes whose sigma fits one tile (every lane loading, no
+// serialisation of the ranks over the warps): 144.8 -> 149.5 ms at c3, 4.4 -> 4.8 ms at c2 (three shared-memory atomics per item).
 int hh_far_apply(hh_ctx* ctx) {
   if (ctx->res_next <= ctx->res_first) return HH_OK;
   cudaStream_t s = ctx->stream;

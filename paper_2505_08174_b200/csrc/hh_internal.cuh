@@ -82,6 +82,8 @@ struct hh_ctx {
   DevScalars* d_sc;
   float *w2, *w3;                       /* packed weights                                     */
   float* w2tc;                          /* W2 as the tensor-core B operand: tf32 hi | lo, core-matrix layout (near_path 1, 2) */
+  int mlp2_wide;                        /* the two-body MLP is the paper-size 4-128-512-128-9 (hh_wide.cuh)  */
+  float* w2w;                           /* its packed weights (hh_pack_wide)                                    */
   double* w2d;                          /* the two-body weights as fp64 (aca_precision = 1)   */
   u64 *keys[2]; u32 *idx[2];            /* radix ping-pong                                    */
   u32* hist;  size_t hist_cap;          /* radix histograms / generic scan tile sums          */
@@ -138,6 +140,10 @@ int hh_sort_pairs(hh_ctx* ctx, u64* keys[2], u32* vals[2], int64_t n, int bit_lo
 int hh_tree_build(hh_ctx* ctx, const float* X, int64_t N);
 int hh_blocks_build(hh_ctx* ctx);
 int hh_near_apply(hh_ctx* ctx);                                       /* Us += near-field           */
+int hh_near_apply_wide(hh_ctx* ctx);                                  /* paper-size MLP (hh_wide.cu) */
+int hh_entries_eval_wide(hh_ctx* ctx, const float* Xi, const float* Xj, int64_t n, float* M);
+int hh_pack_wide(hh_ctx* ctx, const hh_mlp* m, float* out);
+size_t hh_wide_floats(void);
 int hh_near_apply_tc(hh_ctx* ctx);                                    /* the same on tcgen05 tensor cores (hh_near_tc.cu) */
 void hh_pack_w2_tc(const float* W2, float* out);                      /* host: W2 [32][32] -> 2 x 1024 floats */
 int hh_dense_apply(hh_ctx* ctx);                                      /* Us += resident blocks on which ACA broke down, densely */

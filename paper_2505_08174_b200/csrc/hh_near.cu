@@ -85,6 +85,7 @@ __global__ void __launch_bounds__(NR_T, 2) k_near(const float* __restrict__ gw, 
 
 int hh_near_apply(hh_ctx* ctx) {
   if (ctx->n_leaves <= 0 || ctx->nH <= 0) return HH_OK;
+  if (ctx->mlp2_wide) return hh_near_apply_wide(ctx);
   if (ctx->p.near_path != 0) return hh_near_apply_tc(ctx);
   k_near<<<HH_N + ctx->n_leaves, NR_T, 0, ctx->stream>>>(ctx->w2, ctx->p.radius_a, ctx->leaf_nodes, ctx->nlo, ctx->nhi, ctx->PH,
                                                   ctx->near_begin, ctx->near_end, ctx->Xs, ctx->Fs, ctx->Us);

@@ -11,5 +11,5 @@ from .rng import splitmix64, uniform01, normal01  # noqa: F401
 from .generators import (  # noqa: F401
     cube_cloud, ball_cloud, chain_cloud, lattice_cloud, line_points, lattice_drop, two_drops, filament_sphere, mixture_forces,
     gaussian_forces, gravity_forces, filament_forces,
-    xavier_mlp, MLP2_DIMS, MLP3_DIMS, config, CONFIGS,
+    xavier_mlp, MLP2_DIMS, MLP3_DIMS, MLP2_PAPER_DIMS, config, CONFIGS,
 )

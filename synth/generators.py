@@ -10,6 +10,7 @@ from .rng import uniform01, normal01
 
 MLP2_DIMS = (4, 32, 32, 9)    # two-body: [r_hat(3), a/r] -> 3x3   (BASELINE.json configs)
 MLP3_DIMS = (7, 64, 64, 9)    # three-body: [r_ij(3), r_ik(3), |r_jk|] -> 3x3
+MLP2_PAPER_DIMS = (4, 128, 512, 128, 9)   # the paper's hidden layers 128 / 512 / 128 on the configs' features / outputs
 
 
 # ----------------------------------------------------------------------------- positions

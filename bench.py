@@ -32,7 +32,7 @@ UNIT = "particles/s"
 FAR_BYTES_PER_UNIT = 36          # bytes of fp32 factors read per (row or column) x block-rank (DESIGN.md far-field)
 # dram__bytes_read.sum + dram__bytes_write.sum of the k_far launches / their algorithmic factor bytes, from the ncu --set full
 # capture summarised in profiles/r02_far_traffic_c3.md (per launch; the bench line scales it to the launches of one step)
-FAR_TRAFFIC_RATIO = None
+FAR_TRAFFIC_RATIO = 1.063
 ORACLE_SAMPLE_N = {"c1": 2048, "c2": 8192, "c3": 24576, "c4": 16384, "c5": 16000, "p1": 60000, "p2": 60000}
 
 

@@ -94,6 +94,21 @@ def three_body(X, F, mlp3, rcut, brute=False):
     return U, int(nf.value)
 
 
+def self_terms(X, F, mlp2, mlp3, rcut, a=1.0):
+    """The diagonal terms M^(s,2) F + M^(s,3) F of Eq. (6) from the self halves (first 9 outputs) of
+    18-output networks; a network with 9 outputs (or None) contributes nothing.  Returns (U, n_pairs, n_faces)."""
+    X = np.ascontiguousarray(X, np.float32)
+    F = np.ascontiguousarray(F, np.float32)
+    N = X.shape[0]
+    U = np.zeros((N, 3), np.float64)
+    d2, n2, f2 = pack_mlp(*mlp2) if mlp2 is not None else (None, 0, None)
+    d3, n3, f3 = pack_mlp(*mlp3) if mlp3 is not None else (None, 0, None)
+    npairs, nf = C.c_int64(0), C.c_int64(0)
+    lib().orc_self_terms(C.c_int64(N), _vp(X), _vp(F), _vp(d2), n2, _vp(f2), _vp(d3), n3, _vp(f3), C.c_double(a), C.c_float(rcut),
+                         _vp(U), C.byref(npairs), C.byref(nf))
+    return U, int(npairs.value), int(nf.value)
+
+
 def morton_keys(X):
     X = np.ascontiguousarray(X, np.float32)
     keys = np.zeros(X.shape[0], np.uint64)

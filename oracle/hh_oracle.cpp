@@ -87,7 +87,19 @@ void entry2(const Mlp& m, double a, const float* Xi, const float* Xj, double M[9
   double d = std::sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
   if (d < 1e-12 * a) d = 1e-12 * a;
   double x[4] = {r[0] / d, r[1] / d, r[2] / d, a / d};
-  double y[9];
+  double y[18];
+  mlp_forward(m, x, y);
+  // an 18-output network emits alpha_2 = [alpha_2^(s), alpha_2^(t)] (Eq. (2)): the H-matrix holds the transverse half
+  const int off = m.dims[m.nl] == 18 ? 9 : 0;
+  for (int t = 0; t < 9; ++t) M[t] = y[off + t] / d;
+}
+// the self half alpha_2^(s)(X_i, X_j) of an 18-output network (same normalisation, Eq. (4))
+void entry2_self(const Mlp& m, double a, const float* Xi, const float* Xj, double M[9]) {
+  double r[3] = {(double)Xj[0] - (double)Xi[0], (double)Xj[1] - (double)Xi[1], (double)Xj[2] - (double)Xi[2]};
+  double d = std::sqrt(r[0] * r[0] + r[1] * r[1] + r[2] * r[2]);
+  if (d < 1e-12 * a) d = 1e-12 * a;
+  double x[4] = {r[0] / d, r[1] / d, r[2] / d, a / d};
+  double y[18];
   mlp_forward(m, x, y);
   for (int t = 0; t < 9; ++t) M[t] = y[t] / d;
 }
@@ -108,8 +120,10 @@ inline bool within_cut_f32(const float* A, const float* B, float rcut) {
 }
 
 // S-23: U_i += R(MLP3([X_j-X_i, X_k-X_i, |X_j-X_k|])) F_j / (|X_j-X_k| |X_k-X_i|)  (Eq. (4))
+// An 18-output three-body network emits [alpha_3^(s), alpha_3^(t)] (L56): `self` selects the first half (it then multiplies F_i,
+// passed in place of F_j), otherwise the transverse half (or the 9 outputs of a 9-output network) multiplies F_j.
 void face_term(const Mlp& m3, const float* Xi, const float* Xj, const float* Xk, const float* Fj,
-               double* u) {
+               double* u, bool self = false) {
   double x[7], djk = 0, dki = 0;
   for (int c = 0; c < 3; ++c) {
     x[c] = (double)Xj[c] - (double)Xi[c];
@@ -121,8 +135,9 @@ void face_term(const Mlp& m3, const float* Xi, const float* Xj, const float* Xk,
   djk = std::sqrt(djk);
   dki = std::sqrt(dki);
   x[6] = djk;
-  double y[9];
-  mlp_forward(m3, x, y);
+  double yy[18];
+  mlp_forward(m3, x, yy);
+  const double* y = yy + ((!self && m3.dims[m3.nl] == 18) ? 9 : 0);
   double s = 1.0 / (djk * dki);
   double f[3] = {(double)Fj[0], (double)Fj[1], (double)Fj[2]};
   for (int al = 0; al < 3; ++al) u[al] += s * (y[3 * al] * f[0] + y[3 * al + 1] * f[1] + y[3 * al + 2] * f[2]);
@@ -731,6 +746,54 @@ void orc_three_body(int64_t N, const float* X, const float* F, const int* dims, 
         ++nf;
       }
   }
+  if (n_faces) *n_faces = nf;
+}
+
+// The diagonal (self) terms of Eq. (6):  U_i += [ M^(s,2)_ii + M^(s,3)_ii ] F_i  with
+//   M^(s,2)_ii = sum_{j != i, |X_j - X_i| < R_cut} alpha_2^(s)(X_i, X_j)          (Eq. (2); cutoff L56)
+//   M^(s,3)_ii = sum_{faces (j,k,i): i, j in N(k), j != i} alpha_3^(s)(X_i, X_k, X_j)
+// from the first 9 outputs of the 18-output networks.  Plain loops: every N(k) by an O(N) scan.  U += .
+void orc_self_terms(int64_t N, const float* X, const float* F, const int* dims2, int nl2, const float* params2,
+                    const int* dims3, int nl3, const float* params3, double a, float rcut, double* U,
+                    int64_t* n_pairs, int64_t* n_faces) {
+  int64_t np = 0, nf = 0;
+  if (dims2 && dims2[nl2] == 18) {
+    Mlp m2 = make_mlp(dims2, nl2, params2);
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : np)
+    for (int64_t i = 0; i < N; ++i) {
+      double S[9] = {0};
+      for (int64_t j = 0; j < N; ++j) {
+        if (j == i || !within_cut_f32(X + 3 * j, X + 3 * i, rcut)) continue;
+        double M[9];
+        entry2_self(m2, a, X + 3 * i, X + 3 * j, M);
+        for (int t = 0; t < 9; ++t) S[t] += M[t];
+        ++np;
+      }
+      for (int al = 0; al < 3; ++al)
+        U[3 * i + al] += S[3 * al] * (double)F[3 * i] + S[3 * al + 1] * (double)F[3 * i + 1] + S[3 * al + 2] * (double)F[3 * i + 2];
+    }
+  }
+  if (dims3 && dims3[nl3] == 18) {
+    Mlp m3 = make_mlp(dims3, nl3, params3);
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : nf)
+    for (int64_t k = 0; k < N; ++k) {
+      std::vector<int64_t> nb;
+      for (int64_t p = 0; p < N; ++p)
+        if (p != k && within_cut_f32(X + 3 * p, X + 3 * k, rcut)) nb.push_back(p);
+      for (int64_t i : nb)
+        for (int64_t j : nb) {
+          if (i == j) continue;
+          double u[3] = {0, 0, 0};
+          face_term(m3, X + 3 * i, X + 3 * j, X + 3 * k, F + 3 * i, u, true);
+          for (int c = 0; c < 3; ++c) {
+#pragma omp atomic
+            U[3 * i + c] += u[c];
+          }
+          ++nf;
+        }
+    }
+  }
+  if (n_pairs) *n_pairs = np;
   if (n_faces) *n_faces = nf;
 }
 

@@ -217,3 +217,86 @@ def test_zero_force_means_zero_velocity(mlp2_bias, mlp3):
     F = np.zeros((40, 3), np.float32)
     assert np.all(oracle.dense_matvec(X, F, mlp2_bias) == 0)
     assert np.all(oracle.three_body(X, F, mlp3, 4.0)[0] == 0)
+
+
+# ---- self terms M^(s,2), M^(s,3) of Eq. (6) (Eq. (2)): 18-output networks [alpha^(s), alpha^(t)] ----
+def _np_mlp(mlp, x):
+    """numpy restatement of y = W_L tanh(... tanh(W_1 x + b_1) ...) + b_L, independent of the oracle's code"""
+    Ws, bs = mlp
+    h = np.asarray(x, np.float64)
+    for l, (W, b) in enumerate(zip(Ws, bs)):
+        h = W.astype(np.float64) @ h + b.astype(np.float64)
+        if l + 1 < len(Ws):
+            h = np.tanh(h)
+    return h
+
+
+def test_self_terms_against_numpy_brute_force():
+    import synth
+    n, rcut = 36, 4.0
+    X = synth.cube_cloud(n, 0.15, seed=8)
+    F = synth.gaussian_forces(n, seed=9)
+    m2 = synth.xavier_mlp((4, 32, 32, 18), 1, bias_scale=0.2)
+    m3 = synth.xavier_mlp((7, 64, 64, 18), 3, bias_scale=0.2)
+    U, npairs, nf = oracle.self_terms(X, F, m2, m3, rcut)
+    Xd, Fd = X.astype(np.float64), F.astype(np.float64)
+    inside = lambda p, q: np.float32(((X[p] - X[q]) ** 2).sum()) < np.float32(rcut * rcut)
+    ref = np.zeros((n, 3))
+    cnt2 = cnt3 = 0
+    for i in range(n):
+        for j in range(n):
+            if j == i or not inside(j, i):
+                continue
+            r = Xd[j] - Xd[i]
+            d = np.linalg.norm(r)
+            y = _np_mlp(m2, [r[0] / d, r[1] / d, r[2] / d, 1.0 / d])
+            ref[i] += (y[:9].reshape(3, 3) / d) @ Fd[i]                    # alpha_2^(s) acts on F_i
+            cnt2 += 1
+    for k in range(n):
+        nb = [p for p in range(n) if p != k and inside(p, k)]
+        for i in nb:
+            for j in nb:
+                if i == j:
+                    continue
+                djk, dki = np.linalg.norm(Xd[j] - Xd[k]), np.linalg.norm(Xd[k] - Xd[i])
+                y = _np_mlp(m3, np.concatenate([Xd[j] - Xd[i], Xd[k] - Xd[i], [djk]]))
+                ref[i] += (y[:9].reshape(3, 3) / (djk * dki)) @ Fd[i]        # alpha_3^(s) acts on F_i
+                cnt3 += 1
+    assert (npairs, nf) == (cnt2, cnt3) and cnt2 > 0 and cnt3 > 0
+    assert rel_l2(U, ref) < 1e-12
+
+
+def test_self_terms_special_cases():
+    import synth
+    n, rcut = 60, 5.0
+    X = synth.cube_cloud(n, 0.1, seed=2)
+    F = synth.gaussian_forces(n, seed=3)
+    # 9-output networks have no self half: nothing is added
+    U0, p0, f0 = oracle.self_terms(X, F, synth.xavier_mlp((4, 32, 32, 9), 1), synth.xavier_mlp((7, 64, 64, 9), 3), rcut)
+    assert np.all(U0 == 0) and (p0, f0) == (0, 0)
+    # all weights zero, b_last = [vec(I), anything]: alpha_2^(s) = I / r, so U_i = F_i * sum_{j in N(i)} 1 / r_ij (closed form)
+    Ws, bs = zero_mlp((4, 32, 32, 18), b_last=np.concatenate([np.eye(3).ravel(), np.full(9, 7.0)]))
+    U1, p1, _ = oracle.self_terms(X, F, (Ws, bs), None, rcut)
+    D = np.linalg.norm(X[:, None, :].astype(np.float64) - X[None, :, :].astype(np.float64), axis=-1)
+    inside = (((X[:, None, :] - X[None, :, :]) ** 2).sum(-1).astype(np.float32) < np.float32(rcut * rcut)) & ~np.eye(n, dtype=bool)
+    s = np.where(inside, 1.0 / np.where(D > 0, D, 1.0), 0.0).sum(1)
+    assert p1 == int(inside.sum()) and rel_l2(U1, F.astype(np.float64) * s[:, None]) < 1e-13
+    # the transverse half of an 18-output network is what the H-matrix entry and the three-body term use: with the halves swapped
+    # in the last layer the entry of one network is the self entry of the other
+    m2 = synth.xavier_mlp((4, 32, 32, 18), 1, bias_scale=0.1)
+    Wsw = [w.copy() for w in m2[0]]; bsw = [b.copy() for b in m2[1]]
+    Wsw[-1] = np.concatenate([m2[0][-1][9:], m2[0][-1][:9]]); bsw[-1] = np.concatenate([m2[1][-1][9:], m2[1][-1][:9]])
+    m9 = (m2[0][:-1] + [m2[0][-1][9:]], m2[1][:-1] + [m2[1][-1][9:]])
+    assert np.array_equal(oracle.entry2(m2, 1.0, X[0], X[1]), oracle.entry2(m9, 1.0, X[0], X[1]))
+    Ua, _, _ = oracle.self_terms(X, F, (Wsw, bsw), None, rcut)
+    ref = np.zeros((n, 3))
+    for i in range(n):
+        for j in np.flatnonzero(inside[i]):
+            ref[i] += oracle.entry2(m9, 1.0, X[i], X[j]) @ F[i].astype(np.float64)
+    assert rel_l2(Ua, ref) < 1e-13
+    # three-body: the transverse half of an 18-output network equals the 9-output network made of that half
+    m3 = synth.xavier_mlp((7, 64, 64, 18), 3, bias_scale=0.1)
+    m3t = (m3[0][:-1] + [m3[0][-1][9:]], m3[1][:-1] + [m3[1][-1][9:]])
+    Ut, nft = oracle.three_body(X, F, m3, rcut)
+    Ut9, nf9 = oracle.three_body(X, F, m3t, rcut)
+    assert nft == nf9 and np.array_equal(Ut, Ut9)

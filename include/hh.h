@@ -49,7 +49,9 @@ typedef struct hh_ctx hh_ctx;           /* opaque, owned by the library */
 
 /* An MLP  y = W_L tanh( ... tanh(W_1 x + b_1) ... ) + b_L  (tanh on hidden layers only; PAPER.md L92,
  * S-4).  Supported shapes: two-body 4->32->32->9 (features [r_hat(3), a/r], Eq. (4) L85 + config),
- * three-body 7->64->64->9 (features [X_j-X_i, X_k-X_i, |X_j-X_k|]); and, for the two-body term, the paper-size network
+ * three-body 7->64->64->9 (features [X_j-X_i, X_k-X_i, |X_j-X_k|]); either may have 18 outputs instead of 9 = [alpha^(s), alpha^(t)]
+ * (Eq. (2)): the last 9 are the transverse half used above, the first 9 the self half of the diagonal terms M^(s,2), M^(s,3) of
+ * Eq. (6) (L108-L113), summed over the neighbours within rcut3 and applied to F_i; and, for the two-body term, the paper-size network
  * 4->128->512->128->9 (n_layers = 4; L92), evaluated on the tcgen05 tensor cores with tf32 operands and tanh.approx
  * (tolerance 2e-3; meant for the paper's own ACA tolerances zeta >= 1e-2; lock-step ACA only, no S-18b, no parity mode).
  *   dims : HOST   int32[n_layers+1]
@@ -68,7 +70,7 @@ typedef struct {
   float   aca_tol;       /* zeta of Eq. (10)                                                 */
   int32_t aca_max_rank;  /* N_ite_max (L258): cap on the block-rank l; 1..96                       */
   float   radius_a;      /* particle radius a (L41)                                                */
-  float   rcut3;         /* three-body cutoff R_cut (L90); 0 = no three-body term                  */
+  float   rcut3;         /* R_cut of the short-range terms (three-body and self terms; L56, L90); 0 = none */
   int32_t pivot_rule;    /* 0 = |det| (Eq. (9)), 1 = Frobenius (listing L219/L224); S-18 */
   int32_t near_path;     /* near-field entry evaluation (rows 6, 8): 0 = fp32 ALU path (tolerance 1e-5).  1 = tcgen05 tensor cores:
                             the 32 x 32 layer as a tf32 contraction with the accumulator in tensor memory, tanh.approx
@@ -108,6 +110,7 @@ typedef struct {
   float   pad_;
   int64_t n_launches;                      /* kernels launched since the last hh_build_tree began (one whole hh_step) */
   int64_t fallback_entries;                /* sum |tau||sigma| over the blocks counted in aca_singular (dense evaluations per mat-vec) */
+  int64_t n_self_pairs;                    /* pairs (i, j in N(i)) visited by the two-body self term M^(s,2) (Eq. (6))                  */
 } hh_stats;
 
 /* Create a context.  params: HOST.  mlp2: HOST struct, required.  mlp3: HOST struct or NULL (then
@@ -155,7 +158,8 @@ int hh_aca(hh_ctx* ctx, int64_t first_block, int64_t* next_block);
  * Errors: NOT_BUILT, CUDA, WORKSPACE_TOO_SMALL. */
 int hh_matvec(hh_ctx* ctx, const float* F, float* U);
 
-/* Selective mat-vec for tests and stage timing: bit 0 self, 1 near, 2 far, 3 three-body. */
+/* Selective mat-vec for tests and stage timing: bit 0 alpha_1 = I, 1 near, 2 far, 3 three-body M^(t,3), 4 the diagonal self terms
+ * M^(s,2) + M^(s,3) (present only with 18-output networks).  hh_matvec = all five. */
 int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts);
 
 /* Far-field apply only, over the factors currently in the arena (blocks [first, next) of the last

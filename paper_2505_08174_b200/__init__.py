@@ -48,7 +48,7 @@ class Stats(C.Structure):
                  "far_rows_cols", "sum_rank", "aca_entries", "factor_bytes", "aca_batches", "aca_not_converged",
                  "aca_singular", "n_faces", "workspace_required", "arena_bytes")] + \
                [(n, C.c_float) for n in ("ms_tree", "ms_blocks", "ms_aca", "ms_near", "ms_far", "ms_three", "ms_other", "pad_")] + \
-               [("n_launches", C.c_int64), ("fallback_entries", C.c_int64)]
+               [("n_launches", C.c_int64), ("fallback_entries", C.c_int64), ("n_self_pairs", C.c_int64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -170,7 +170,7 @@ class Context:
         self._chk(self.lib.hh_aca(self._h, C.c_int64(first_block), C.byref(nxt)))
         return int(nxt.value)
 
-    def matvec(self, F, U=None, parts=15):
+    def matvec(self, F, U=None, parts=31):
         if U is None:
             U = self.torch.empty_like(F)
         self._chk(self.lib.hh_matvec_parts(self._h, _ptr(F), _ptr(U), int(parts)))

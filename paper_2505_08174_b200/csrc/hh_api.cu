@@ -33,6 +33,8 @@ static int carve(hh_ctx* ctx, int64_t N) {
   ctx->d_sc = c.take<DevScalars>(1);
   ctx->w2 = c.take<float>(HH_MLP2_FLOATS);
   ctx->w3 = c.take<float>(HH_MLP3_FLOATS);
+  ctx->w2s = c.take<float>(HH_MLP2_FLOATS);
+  ctx->w3s = c.take<float>(HH_MLP3_FLOATS);
   ctx->w2d = c.take<double>(HH_MLP2_FLOATS);
   ctx->w2tc = c.take<float>(2 * 1024);
   ctx->w2w = c.take<float>(hh_wide_floats());
@@ -85,10 +87,13 @@ static int check_params(const hh_params* p) {
 }
 
 // copy an MLP to the host and pack it as MlpOff<INP,H> describes (input dim zero-padded to INP)
-static int pack_mlp(hh_ctx* ctx, const hh_mlp* m, int in, int INP, int H, std::vector<float>& out) {
+// An 18-output network emits [alpha^(s), alpha^(t)] (Eq. (2)): `out` receives the transverse half (outputs 9..17, what the
+// H-matrix and the transverse three-body term use), `out_self` the self half (outputs 0..8) as a second 9-output weight set.
+static int pack_mlp(hh_ctx* ctx, const hh_mlp* m, int in, int INP, int H, std::vector<float>& out, std::vector<float>* out_self = nullptr) {
   if (m->n_layers != 3 || !m->dims || !m->W || !m->b) return HH_ERR_UNSUPPORTED;
-  if (m->dims[0] != in || m->dims[1] != H || m->dims[2] != H || m->dims[3] != 9) return HH_ERR_UNSUPPORTED;
-  std::vector<float> W1((size_t)H * in), b1(H), W2((size_t)H * H), b2(H), W3((size_t)9 * H), b3(9);
+  if (m->dims[0] != in || m->dims[1] != H || m->dims[2] != H || (m->dims[3] != 9 && m->dims[3] != 18)) return HH_ERR_UNSUPPORTED;
+  const int nout = m->dims[3], off = nout == 18 ? 9 : 0;
+  std::vector<float> W1((size_t)H * in), b1(H), W2((size_t)H * H), b2(H), W3((size_t)nout * H), b3(nout);
   float* dst[6] = {W1.data(), b1.data(), W2.data(), b2.data(), W3.data(), b3.data()};
   const float* src[6] = {m->W[0], m->b[0], m->W[1], m->b[1], m->W[2], m->b[2]};
   size_t cnt[6] = {W1.size(), b1.size(), W2.size(), b2.size(), W3.size(), b3.size()};
@@ -107,9 +112,13 @@ static int pack_mlp(hh_ctx* ctx, const hh_mlp* m, int in, int INP, int H, std::v
   o += (size_t)H * H;
   for (int r = 0; r < H; ++r) out[o + r] = b2[r];
   o += H;
-  for (int h = 0; h < H; ++h) for (int r = 0; r < 9; ++r) out[o + (size_t)h * 12 + r] = W3[(size_t)r * H + h];
+  if (out_self) { out_self->clear(); if (nout == 18) *out_self = out; }
+  for (int h = 0; h < H; ++h) for (int r = 0; r < 9; ++r) out[o + (size_t)h * 12 + r] = W3[(size_t)(off + r) * H + h];
+  if (out_self && nout == 18)
+    for (int h = 0; h < H; ++h) for (int r = 0; r < 9; ++r) (*out_self)[o + (size_t)h * 12 + r] = W3[(size_t)r * H + h];
   o += (size_t)H * 12;
-  for (int r = 0; r < 9; ++r) out[o + r] = b3[r];
+  for (int r = 0; r < 9; ++r) out[o + r] = b3[off + r];
+  if (out_self && nout == 18) for (int r = 0; r < 9; ++r) (*out_self)[o + r] = b3[r];
   return HH_OK;
 }
 
@@ -148,7 +157,7 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   *out = nullptr;
   if (!check_params(params) || !mlp2 || !workspace) return HH_ERR_INVALID_ARG;
   if (((uintptr_t)workspace & 255) != 0) return HH_ERR_INVALID_ARG;
-  if (!mlp3 && params->rcut3 > 0.f) return HH_ERR_INVALID_ARG;
+  if (!mlp3 && params->rcut3 > 0.f && !(mlp2->n_layers == 3 && mlp2->dims && mlp2->dims[3] == 18)) return HH_ERR_INVALID_ARG;
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return HH_ERR_CUDA; }   // no CPU fallback
   hh_ctx* ctx = new (std::nothrow) hh_ctx();
@@ -185,8 +194,13 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
     HH_CUDA(cudaStreamSynchronize(ctx->stream));
     ctx->mlp2_wide = 1;
   } else {
-  r = pack_mlp(ctx, mlp2, 4, HH_MLP2_INP, HH_MLP2_H, pk);
-  if (r != HH_OK) return hh_fail(ctx, r, "two-body MLP must be 4->32->32->9 (or 4->128->512->128->9) with device weight pointers");
+  std::vector<float> pks;
+  r = pack_mlp(ctx, mlp2, 4, HH_MLP2_INP, HH_MLP2_H, pk, &pks);
+  if (r != HH_OK) return hh_fail(ctx, r, "two-body MLP must be 4->32->32->9 / 18 (or 4->128->512->128->9) with device weight pointers");
+  if (!pks.empty()) {
+    HH_CUDA(cudaMemcpyAsync(ctx->w2s, pks.data(), pks.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+    ctx->have_self2 = 1;
+  }
   HH_CUDA(cudaMemcpyAsync(ctx->w2, pk.data(), pk.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
   std::vector<double> pkd(pk.begin(), pk.end());
   std::vector<float> w2tc(2 * 1024);
@@ -196,8 +210,14 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   HH_CUDA(cudaStreamSynchronize(ctx->stream));
   }
   if (mlp3) {
-    r = pack_mlp(ctx, mlp3, 7, HH_MLP3_INP, HH_MLP3_H, pk);
-    if (r != HH_OK) return hh_fail(ctx, r, "three-body MLP must be 7->64->64->9 with device weight pointers");
+    std::vector<float> pks3;
+    r = pack_mlp(ctx, mlp3, 7, HH_MLP3_INP, HH_MLP3_H, pk, &pks3);
+    if (r != HH_OK) return hh_fail(ctx, r, "three-body MLP must be 7->64->64->9 / 18 with device weight pointers");
+    if (!pks3.empty()) {
+      HH_CUDA(cudaMemcpyAsync(ctx->w3s, pks3.data(), pks3.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+      HH_CUDA(cudaStreamSynchronize(ctx->stream));
+      ctx->have_self3 = 1;
+    }
     HH_CUDA(cudaMemcpyAsync(ctx->w3, pk.data(), pk.size() * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
     HH_CUDA(cudaStreamSynchronize(ctx->stream));
     ctx->have_mlp3 = 1;
@@ -217,7 +237,7 @@ extern "C" int hh_destroy(hh_ctx* ctx) {
 extern "C" int hh_set_params(hh_ctx* ctx, const hh_params* params) {
   if (!ctx) return HH_ERR_INVALID_ARG;
   if (!check_params(params)) return hh_fail(ctx, HH_ERR_INVALID_ARG, "invalid parameters");
-  if (params->rcut3 > 0.f && !ctx->have_mlp3) return hh_fail(ctx, HH_ERR_INVALID_ARG, "rcut3 > 0 needs a three-body MLP");
+  if (params->rcut3 > 0.f && !ctx->have_mlp3 && !ctx->have_self2) return hh_fail(ctx, HH_ERR_INVALID_ARG, "rcut3 > 0 needs a three-body MLP or an 18-output two-body MLP");
   if (ctx->mlp2_wide && (params->kappa_max > 0.f || params->aca_precision != 0))
     return hh_fail(ctx, HH_ERR_UNSUPPORTED, "the paper-size MLP path has neither the S-18b dense fallback nor the fp64 parity mode");
   if (params->leaf_size != ctx->p.leaf_size) ctx->tree_ok = ctx->blocks_ok = 0;
@@ -365,9 +385,10 @@ extern "C" int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts)
       }
     }
   }
-  if ((parts & 8) && ctx->p.rcut3 > 0.f) {
+  const int short_modes = ((parts & 8) && ctx->have_mlp3 ? 1 : 0) | ((parts & 16) ? 6 : 0);
+  if (short_modes && ctx->p.rcut3 > 0.f) {
     T0(4);
-    HH_TRY(hh_three_apply(ctx));
+    HH_TRY(hh_three_apply(ctx, short_modes));
     T0(5);
     if (ctx->timing) ctx->st.ms_three = ev_ms(ctx, 4, 5);
   }
@@ -379,7 +400,7 @@ extern "C" int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts)
   return HH_OK;
 }
 
-extern "C" int hh_matvec(hh_ctx* ctx, const float* F, float* U) { return hh_matvec_parts(ctx, F, U, 15); }
+extern "C" int hh_matvec(hh_ctx* ctx, const float* F, float* U) { return hh_matvec_parts(ctx, F, U, 31); }
 
 extern "C" int hh_far_apply_resident(hh_ctx* ctx, const float* F, float* U) {
   if (!ctx) return HH_ERR_INVALID_ARG;

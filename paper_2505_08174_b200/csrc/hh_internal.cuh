@@ -49,6 +49,7 @@ struct DevScalars {
   u64 near_entries, far_rows_cols;
   u32 max_rank_seen, n_dense;
   u64 fallback_entries;
+  u64 n_self_pairs;         /* pairs (i, j in N(i)) visited by the two-body self term */
   u64 cap_count;            /* pivot records written by hh_set_capture's kernel (may exceed the caller's capacity) */
   u64 batch_units, batch_units1;  /* lock-step ACA: padded rows + columns of the batch [first, batch_end) resp. of block `first` alone */
 };
@@ -81,6 +82,8 @@ struct hh_ctx {
   /* carved device pointers */
   DevScalars* d_sc;
   float *w2, *w3;                       /* packed weights                                     */
+  float *w2s, *w3s;                     /* self halves of 18-output networks, packed as 9-output sets (Eq. (2)) */
+  int have_self2, have_self3;
   float* w2tc;                          /* W2 as the tensor-core B operand: tf32 hi | lo, core-matrix layout (near_path 1, 2) */
   int mlp2_wide;                        /* the two-body MLP is the paper-size 4-128-512-128-9 (hh_wide.cuh)  */
   float* w2w;                           /* its packed weights (hh_pack_wide)                                    */
@@ -151,7 +154,7 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next);      /* one CTA per
 int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next);     /* lock-step over the batch (hh_aca2.cu) */
 int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next);   /* stats, dense list, rank prediction */
 int hh_far_apply(hh_ctx* ctx);                                        /* Us += resident far-field   */
-int hh_three_apply(hh_ctx* ctx);                                     /* Us += three-body term (tree order) */
+int hh_three_apply(hh_ctx* ctx, int modes);                          /* Us += short-range terms (tree order): bit 0 M^(t,3), 1 M^(s,3), 2 M^(s,2) */
 int hh_entries_eval(hh_ctx* ctx, const float* Xi, const float* Xj, int64_t n, float* M);
 int hh_factors_fetch(hh_ctx* ctx, int64_t block, int32_t* rank, int32_t* flag, int32_t cap_rank,
                      int32_t* piv_i, int32_t* piv_j, float* C, float* Q);

@@ -47,14 +47,19 @@ __device__ __forceinline__ bool within_cut(const float* A, const float* B, float
   return d2 < rc2;
 }
 
-__global__ void __launch_bounds__(TB_T) k_three(const float* __restrict__ gw, const float* __restrict__ Xs, const float* __restrict__ Fs,
+// MODE 0: the transverse three-body term M^(t,3) (row 10).  MODE 1: the three-body SELF term M^(s,3) of Eq. (6) (L108-L113): the same
+// faces, the self half of the 18-output network (packed as a second 9-output weight set), acting on F_i.  MODE 2: the two-body SELF
+// term M^(s,2): U_k += [ sum_{j in N(k)} alpha_2^(s)(X_k, X_j) ] F_k, the self half of the 18-output two-body network on the same
+// neighbour lists (Eq. (2); all three cut-off terms share R_cut, L56).
+template <int MODE>
+__global__ void __launch_bounds__(TB_T) k_three(const float* __restrict__ gw, float a, const float* __restrict__ Xs, const float* __restrict__ Fs,
                                                  float* __restrict__ Us, int64_t N, CellGrid G, const u32* __restrict__ cell_start,
                                                  const u32* __restrict__ order, float rcut, DevScalars* sc) {
   extern __shared__ __align__(16) float dyn[];
-  float* sw = dyn;                                               // HH_MLP3_FLOATS
+  float* sw = dyn;                                               // HH_MLP3_FLOATS (MODE 2: HH_MLP2_FLOATS used)
   u32* nbl = (u32*)(dyn + HH_MLP3_FLOATS);                       // [warps][TB_CAP]
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  load_weights(sw, gw, HH_MLP3_FLOATS);
+  load_weights(sw, gw, MODE == 2 ? HH_MLP2_FLOATS : HH_MLP3_FLOATS);
   __syncthreads();
   const int64_t k = (int64_t)blockIdx.x * (TB_T / 32) + warp;
   if (k >= N) return;
@@ -88,9 +93,34 @@ __global__ void __launch_bounds__(TB_T) k_three(const float* __restrict__ gw, co
     }
   __syncwarp();
   if (d > TB_CAP) { if (lane == 0) atomicAdd(&sc->deg_overflow, 1u); return; }
+  if (MODE == 2) {
+    if (d < 1) return;
+    if (lane == 0) atomicAdd((unsigned long long*)&sc->n_self_pairs, (unsigned long long)d);
+    float S[9];
+#pragma unroll
+    for (int r = 0; r < 9; ++r) S[r] = 0.f;
+    for (u32 f = lane; f < d; f += 32) {
+      const u32 j = nb[f];
+      float xi[1][3], xj[1][3], M[1][9];
+#pragma unroll
+      for (int c = 0; c < 3; ++c) { xi[0][c] = xk[c]; xj[0][c] = Xs[3 * (size_t)j + c]; }
+      entry2_eval<1>(sw, a, xi, xj, M);
+#pragma unroll
+      for (int r = 0; r < 9; ++r) S[r] += M[0][r];
+    }
+#pragma unroll
+    for (int r = 0; r < 9; ++r)
+#pragma unroll
+      for (int o = 16; o; o >>= 1) S[r] += __shfl_xor_sync(0xffffffffu, S[r], o);
+    if (lane < 3) {
+      const float f0 = Fs[3 * k], f1 = Fs[3 * k + 1], f2 = Fs[3 * k + 2];
+      atomicAdd(&Us[3 * k + lane], fmaf(S[3 * lane], f0, fmaf(S[3 * lane + 1], f1, S[3 * lane + 2] * f2)));
+    }
+    return;
+  }
   if (d < 2) return;
   const u32 nf = d * (d - 1);
-  if (lane == 0) atomicAdd((unsigned long long*)&sc->n_faces, (unsigned long long)nf);
+  if (lane == 0 && MODE == 0) atomicAdd((unsigned long long*)&sc->n_faces, (unsigned long long)nf);
   for (u32 f = lane; f < nf; f += 32) {
     u32 a = f / (d - 1), b = f - a * (d - 1);
     if (b >= a) ++b;
@@ -110,15 +140,20 @@ __global__ void __launch_bounds__(TB_T) k_three(const float* __restrict__ gw, co
     x[0][6] = djk; x[0][7] = 0.f;
     mlp_eval<HH_MLP3_INP, HH_MLP3_H, 1>(sw, x, out);
     const float s = 1.0f / (djk * dki);
-    const float f0 = Fs[3 * (size_t)j], f1 = Fs[3 * (size_t)j + 1], f2 = Fs[3 * (size_t)j + 2];
+    const size_t jf = MODE == 1 ? (size_t)i : (size_t)j;           // the self half multiplies F_i, the transverse half F_j
+    const float f0 = Fs[3 * jf], f1 = Fs[3 * jf + 1], f2 = Fs[3 * jf + 2];
 #pragma unroll
     for (int al = 0; al < 3; ++al)
       atomicAdd(&Us[3 * (size_t)i + al], s * fmaf(out[0][3 * al], f0, fmaf(out[0][3 * al + 1], f1, out[0][3 * al + 2] * f2)));
   }
 }
 
-int hh_three_apply(hh_ctx* ctx) {
-  if (!ctx->have_mlp3) return hh_fail(ctx, HH_ERR_INVALID_ARG, "three-body term needs a three-body MLP");
+// modes: bit 0 transverse three-body (row 10), bit 1 three-body self term, bit 2 two-body self term
+int hh_three_apply(hh_ctx* ctx, int modes) {
+  if ((modes & 1) && !ctx->have_mlp3) return hh_fail(ctx, HH_ERR_INVALID_ARG, "three-body term needs a three-body MLP");
+  if (!ctx->have_self3) modes &= ~2;
+  if (!ctx->have_self2) modes &= ~4;
+  if (!modes) return HH_OK;
   cudaStream_t s = ctx->stream;
   const int64_t N = ctx->N;
   const float rcut = ctx->p.rcut3;
@@ -152,7 +187,8 @@ int hh_three_apply(hh_ctx* ctx) {
     G.inv[c] = (float)(1.0 / cw);
   }
   const u32 ncells = (u32)((int64_t)G.nc[0] * G.nc[1] * G.nc[2]);
-  HH_CUDA(cudaMemsetAsync(&ctx->d_sc->n_faces, 0, sizeof(u64), s));
+  if (modes & 1) HH_CUDA(cudaMemsetAsync(&ctx->d_sc->n_faces, 0, sizeof(u64), s));
+  if (modes & 4) HH_CUDA(cudaMemsetAsync(&ctx->d_sc->n_self_pairs, 0, sizeof(u64), s));
   HH_CUDA(cudaMemsetAsync(&ctx->d_sc->deg_overflow, 0, sizeof(u32), s));
   k_cell_ids<<<HH_N + cdiv(N, 256), 256, 0, s>>>(ctx->Xs, N, G, ctx->keys[1], ctx->idx[1]);
   // sort (cell id, particle) with the radix ping-pong buffers; keys[0] (the Morton keys) must survive, so the
@@ -165,12 +201,21 @@ int hh_three_apply(hh_ctx* ctx) {
   HH_TRY(hh_sort_pairs(ctx, k2, v2, N, 0, bits, &which));
   k_cell_start<<<HH_N + cdiv(N + 1, 256), 256, 0, s>>>(k2[which], N, ncells, ctx->cell_start);
   size_t smem = (size_t)HH_MLP3_FLOATS * sizeof(float) + (TB_T / 32) * TB_CAP * sizeof(u32);
-  if (!ctx->three_smem_set) { HH_CUDA(cudaFuncSetAttribute(k_three, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)); ctx->three_smem_set = 1; }
-  k_three<<<HH_N + cdiv(N, TB_T / 32), TB_T, smem, s>>>(ctx->w3, ctx->Xs, ctx->Fs, ctx->Us, N, G, ctx->cell_start, v2[which], rcut, ctx->d_sc);
+  if (!ctx->three_smem_set) {
+    HH_CUDA(cudaFuncSetAttribute(k_three<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    HH_CUDA(cudaFuncSetAttribute(k_three<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    HH_CUDA(cudaFuncSetAttribute(k_three<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ctx->three_smem_set = 1;
+  }
+  const float a = ctx->p.radius_a;
+  if (modes & 1) k_three<0><<<HH_N + cdiv(N, TB_T / 32), TB_T, smem, s>>>(ctx->w3, a, ctx->Xs, ctx->Fs, ctx->Us, N, G, ctx->cell_start, v2[which], rcut, ctx->d_sc);
+  if (modes & 2) k_three<1><<<HH_N + cdiv(N, TB_T / 32), TB_T, smem, s>>>(ctx->w3s, a, ctx->Xs, ctx->Fs, ctx->Us, N, G, ctx->cell_start, v2[which], rcut, ctx->d_sc);
+  if (modes & 4) k_three<2><<<HH_N + cdiv(N, TB_T / 32), TB_T, smem, s>>>(ctx->w2s, a, ctx->Xs, ctx->Fs, ctx->Us, N, G, ctx->cell_start, v2[which], rcut, ctx->d_sc);
   HH_LAUNCH_CHECK();
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
-  ctx->st.n_faces = (int64_t)ctx->h_sc->n_faces;
+  if (modes & 1) ctx->st.n_faces = (int64_t)ctx->h_sc->n_faces;
+  if (modes & 4) ctx->st.n_self_pairs = (int64_t)ctx->h_sc->n_self_pairs;
   if (ctx->h_sc->deg_overflow) return hh_fail(ctx, HH_ERR_UNSUPPORTED, "three-body: a particle has more than 256 neighbours within R_cut");
   return HH_OK;
 }

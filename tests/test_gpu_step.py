@@ -80,3 +80,41 @@ def test_step_host_matches_device_step(mlp2, mlp3):
     assert rel_l2(Uh.numpy(), Ud) <= 2e-6                 # atomics: summation order only
     assert np.max(np.abs(Xh.numpy() - Xd.cpu().numpy())) <= 1e-5
     ctx.close()
+
+
+def test_self_terms_of_eq6_with_18_output_networks():
+    """networks with 18 outputs [alpha^(s), alpha^(t)] (Eq. (2)).  The transverse halves feed
+    the H-matrix and the three-body term as before; the self halves give the diagonal terms M^(s,2), M^(s,3) of Eq. (6)
+    (L108-L113), summed over the neighbours within R_cut and applied to F_i (`parts` bit 4)."""
+    n, rcut = 3000, 4.0
+    X = synth.ball_cloud(n, 0.2, seed=6)
+    F = synth.gaussian_forces(n, seed=7)
+    m2 = synth.xavier_mlp((4, 32, 32, 18), 1, bias_scale=0.1)
+    m3 = synth.xavier_mlp((7, 64, 64, 18), 3, bias_scale=0.1)
+    ctx = make_ctx(m2, m3, leaf_size=32, eta=1.0, aca_tol=1e-5, rcut3=rcut, ws_mb=2048)
+    ctx.build_tree(to_dev(X))
+    ctx.build_blocks()
+    Us = ctx.matvec(to_dev(F), parts=16).cpu().numpy()
+    st = ctx.stats()
+    Uo, npairs, nfaces = oracle.self_terms(X, F, m2, m3, rcut)
+    assert st["n_self_pairs"] == npairs and npairs > 0 and nfaces > 0
+    print("self terms: rel L2 vs oracle %.3e (%d pairs, %d faces)" % (rel_l2(Us, Uo), npairs, nfaces))
+    assert rel_l2(Us, Uo) <= 1e-5
+    # the transverse three-body term from the transverse half
+    U3 = ctx.matvec(to_dev(F), parts=8).cpu().numpy()
+    U3o, nf = oracle.three_body(X, F, m3, rcut)
+    assert ctx.stats()["n_faces"] == nf == nfaces and rel_l2(U3, U3o) <= 1e-5
+    # everything together against the definition, Eq. (6): alpha_1 F + M^(t,2) F (dense) + M^(s,2) F + M^(t,3) F + M^(s,3) F
+    U = ctx.matvec(to_dev(F)).cpu().numpy()
+    Uall = oracle.dense_matvec(X, F, m2) + U3o + Uo
+    print("Eq. (6), all five terms: rel L2 vs the definition %.3e" % rel_l2(U, Uall))
+    assert rel_l2(U, Uall) <= 1e-4
+    ctx.close()
+    # a two-body network with a self half and no three-body network at all
+    ctx = make_ctx(m2, None, leaf_size=32, eta=1.0, aca_tol=1e-5, rcut3=rcut, ws_mb=1024)
+    ctx.build_tree(to_dev(X))
+    ctx.build_blocks()
+    U2 = ctx.matvec(to_dev(F), parts=16).cpu().numpy()
+    U2o, _, _ = oracle.self_terms(X, F, m2, None, rcut)
+    assert rel_l2(U2, U2o) <= 1e-5
+    ctx.close()

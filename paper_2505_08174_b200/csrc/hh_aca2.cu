@@ -402,16 +402,16 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
 // ---- paper-size MLP: the entries of lines 4 / 7 for all active blocks, 128 per tensor-core tile (8 granules), stored raw
 // in the slot of rank k (gather coordinates -> network inference -> scatter into C / Q) ----
 template <bool COLS>
-__global__ void __launch_bounds__(128) k2_eval_wide(A2Args A, const float* __restrict__ gw, u32 count, u32* __restrict__ err_flag) {
+__global__ void __launch_bounds__(WD_T) k2_eval_wide(A2Args A, const float* __restrict__ gw, u32 count, u32* __restrict__ err_flag) {
   extern __shared__ __align__(1024) unsigned char we_raw[];
   WideSmem& S = *reinterpret_cast<WideSmem*>(we_raw);
   wide_setup(S, gw);
-  const u32 tid = threadIdx.x, l16 = tid & 15;
+  const u32 tid = threadIdx.x, row = tid & 127u, l16 = row & 15;
   const uint2* gl = COLS ? A.gn : A.gm;
   const u32 ntiles = (count + 7) / 8;
   bool alive = true;
   for (u32 tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const u32 gi = 8 * tile + (tid >> 4);
+    const u32 gi = 8 * tile + (row >> 4);
     const bool gv = gi < count;
     const uint2 g = gl[gv ? gi : count - 1];
     const BlkState& s = A.st[g.x];
@@ -431,7 +431,7 @@ __global__ void __launch_bounds__(128) k2_eval_wide(A2Args A, const float* __res
       x[0] = rx * inv; x[1] = ry * inv; x[2] = rz * inv; x[3] = A.a * inv;
     }
     alive = wide_tile(S, gw, x, out) && alive;
-    if (gv && s.status == 0 && idx < len) {
+    if (tid < 128u && gv && s.status == 0 && idx < len) {                  // the result lives in the first warpgroup
       float* dst = chunk_ptr(A, A.tab + (size_t)g.x * HH_TAB_STRIDE, s.k) +
                    (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(s.k % HH_RC) * 9 * np : (size_t)(s.k % HH_RC) * 9 * mp);
 #pragma unroll
@@ -631,10 +631,10 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       const unsigned gr = (g1 < cap ? g1 : cap), gc = (g1 > g2 ? g1 : g2) < cap ? (g1 > g2 ? g1 : g2) : cap;
       if (ctx->mlp2_wide) {
         const unsigned t1 = cdiv(gmc, 8), t2 = cdiv(gnc, 8), nsm = (unsigned)ctx->n_sm;
-        k2_eval_wide<false><<<HH_N + (t1 < nsm ? t1 : nsm), 128, wsm, s>>>(A, ctx->w2w, gmc, &ctx->d_sc->deg_overflow);
+        k2_eval_wide<false><<<HH_N + (t1 < nsm ? t1 : nsm), WD_T, wsm, s>>>(A, ctx->w2w, gmc, &ctx->d_sc->deg_overflow);
         k2_step<false, false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
         k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
-        k2_eval_wide<true><<<HH_N + (t2 < nsm ? t2 : nsm), 128, wsm, s>>>(A, ctx->w2w, gnc, &ctx->d_sc->deg_overflow);
+        k2_eval_wide<true><<<HH_N + (t2 < nsm ? t2 : nsm), WD_T, wsm, s>>>(A, ctx->w2w, gnc, &ctx->d_sc->deg_overflow);
         k2_step<true, false, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
       } else {
       if (ctx->p.aca_precision) k2_step<false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);

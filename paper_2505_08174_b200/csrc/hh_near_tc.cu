@@ -22,6 +22,9 @@
 #include "hh_mlp.cuh"
 
 #define NT_T 128               /* threads per CTA = rows of one MMA tile                                  */
+#ifndef NT_TANH2
+#define NT_TANH2(x) tanh_ex2(x) /* activation of near_path = 2 (-DNT_TANH2=tanhf for the library tanh)     */
+#endif
 #define NT_TILE 256            /* source particles staged per tile                                        */
 #define NT_SPIN_MAX (1u << 24) /* bounded mbarrier spins: a wrong descriptor must not hang the GPU         */
 
@@ -41,6 +44,16 @@ struct NtSmem {
 __device__ __forceinline__ u32 smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ u32 to_tf32(float x) { u32 r; asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(r) : "f"(x)); return r; }
 __device__ __forceinline__ float tanh_mufu(float x) { float y; asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+// tanh x = 1 - 2 / (1 + 2^(2 x log2 e)) with MUFU ex2 and rcp (2 ulp each): ABSOLUTE error ~2e-7 everywhere (the subtraction cancels
+// for small |x|, so the relative error of tiny values is not kept).  Five instructions instead of tanhf's ~20.  Good for the
+// near-field, where an activation feeds a dot product and only its absolute error matters; NOT used inside Alg. 2, where entry
+// errors are amplified by the pivot conditioning.  Saturates correctly: ex2 -> inf gives 1, ex2 -> 0 gives -1.
+__device__ __forceinline__ float tanh_ex2(float x) {
+  float e, r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(e) : "f"(x * 2.8853900817779268f));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(e + 1.0f));
+  return fmaf(r, -2.0f, 1.0f);
+}
 
 // K-major, no-swizzle shared-memory matrix descriptor: 8-row x 16-byte core matrices, the two K-halves of one instruction
 // 128 B apart (leading byte offset), consecutive 8-row groups 1024 B apart (stride byte offset), descriptor version 1.
@@ -133,7 +146,7 @@ __global__ void __launch_bounds__(NT_T) k_near_tc(const float* __restrict__ gw, 
 #pragma unroll
     for (int o = 0; o < 32; ++o) {
       const float pre = __uint_as_float(dr[o]) + S.b2[o];
-      const float t = SPLIT ? tanhf(pre) : tanh_mufu(pre);
+      const float t = SPLIT ? NT_TANH2(pre) : tanh_mufu(pre);
       const float4 wa = *reinterpret_cast<const float4*>(&S.w3t[12 * o]);
       const float4 wb = *reinterpret_cast<const float4*>(&S.w3t[12 * o + 4]);
       const float wc = S.w3t[12 * o + 8];
@@ -200,7 +213,7 @@ __global__ void __launch_bounds__(NT_T) k_near_tc(const float* __restrict__ gw, 
       for (int o = 0; o < 32; ++o) {
         const float4 w = *reinterpret_cast<const float4*>(&S.w1[4 * o]);
         const float pre = fmaf(w.x, x[0], fmaf(w.y, x[1], fmaf(w.z, x[2], fmaf(w.w, x[3], S.b1[o]))));
-        h[o] = SPLIT ? tanhf(pre) : tanh_mufu(pre);
+        h[o] = SPLIT ? NT_TANH2(pre) : tanh_mufu(pre);
       }
       // ---- the previous MMA has read A: wait for it, then publish this tile's A operand ----
       if (pend) { alive = alive && mbar_wait(bar_mma, phase); phase ^= 1u; }

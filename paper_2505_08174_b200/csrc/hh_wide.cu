@@ -5,7 +5,7 @@
 #include <string.h>
 #include "hh_wide.cuh"
 
-#define WN_T 128
+#define WN_T WD_T            /* 256 threads: two warpgroups per 128-entry tile */
 #define WN_TILE 256
 
 struct WideNearSmem {
@@ -69,10 +69,10 @@ __global__ void __launch_bounds__(WN_T) k_near_wide(const float* __restrict__ gw
     }
     __syncthreads();
     const u32 pairs = m * nt;
-    for (u32 p0 = 0; p0 < pairs; p0 += WN_T) {
-      const u32 p = p0 + tid;
-      const bool valid = p < pairs;
-      const u32 pc = valid ? p : 0u;
+    for (u32 p0 = 0; p0 < pairs; p0 += 128) {
+      const u32 p = p0 + (tid & 127u);
+      const bool valid = p < pairs && tid < 128u;                            // the result lives in the first warpgroup
+      const u32 pc = p < pairs ? p : 0u;
       const u32 jj = pc / m, ii = pc - jj * m;
       float x[4], inv, out[9];
       wide_features(&S.tX[3 * ii], &S.sXj[3 * jj], a, x, inv);
@@ -99,15 +99,15 @@ __global__ void __launch_bounds__(WN_T) k_entries_wide(const float* __restrict__
   WideSmem& S = *reinterpret_cast<WideSmem*>(wn_raw);
   wide_setup(S, gw);
   bool alive = true;
-  for (int64_t t0 = (int64_t)blockIdx.x * WN_T; t0 < n; t0 += (int64_t)gridDim.x * WN_T) {
-    const int64_t t = t0 + threadIdx.x;
+  for (int64_t t0 = (int64_t)blockIdx.x * 128; t0 < n; t0 += (int64_t)gridDim.x * 128) {
+    const int64_t t = t0 + (threadIdx.x & 127);
     const int64_t tc = t < n ? t : n - 1;
     float xi[3], xj[3], x[4], inv, out[9];
 #pragma unroll
     for (int c = 0; c < 3; ++c) { xi[c] = Xi[3 * tc + c]; xj[c] = Xj[3 * tc + c]; }
     wide_features(xi, xj, a, x, inv);
     alive = wide_tile(S, gw, x, out) && alive;
-    if (t < n) {
+    if (t < n && threadIdx.x < 128) {
 #pragma unroll
       for (int r = 0; r < 9; ++r) M[9 * t + r] = out[r] * inv;
     }
@@ -180,7 +180,7 @@ int hh_entries_eval_wide(hh_ctx* ctx, const float* Xi, const float* Xj, int64_t 
   const size_t smem = sizeof(WideSmem) + 1024;
   HH_CUDA(cudaFuncSetAttribute(k_entries_wide, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   HH_CUDA(cudaMemsetAsync(&ctx->d_sc->deg_overflow, 0, sizeof(u32), ctx->stream));
-  const unsigned tiles = cdiv(n, WN_T);
+  const unsigned tiles = cdiv(n, 128);
   k_entries_wide<<<HH_N + (tiles < (unsigned)ctx->n_sm ? tiles : (unsigned)ctx->n_sm), WN_T, smem, ctx->stream>>>(ctx->w2w, ctx->p.radius_a, Xi, Xj, n, M,
                                                                                                                    &ctx->d_sc->deg_overflow);
   HH_LAUNCH_CHECK();

@@ -35,6 +35,7 @@
 #define WD_SMALL WD_OFF_W2                          /* everything before the chunks is copied to shared memory once */
 
 #define WD_SPIN_MAX (1u << 24)
+#define WD_T 256                                    /* threads per CTA: two warpgroups on one 128-entry tile */
 
 struct WideSmem {
   float A1[128 * WD_H1];        /* (row r, k): (r/8)*1024 + (k/4)*32 + (r%8)*4 + (k%4)   [8-row groups 4096 B apart]  */
@@ -42,6 +43,7 @@ struct WideSmem {
   float W3c[WD_H3 * WD_NC];     /* (n, kk):    (n/8)*512  + (kk/4)*32 + (n%8)*4 + (kk%4)  [8-row groups 2048 B apart] */
   float A2c[128 * WD_NC];       /* (r, kk):    (r/8)*512  + (kk/4)*32 + (r%8)*4 + (kk%4)                              */
   float small_[WD_SMALL];       /* W1, b1, b2, b3, W4T, b4                                                            */
+  float red[128 * 9];           /* layer-4 partial sums of the second warpgroup                                       */
   unsigned long long bar_mma, bar_w2, bar_w3;
   u32 tmem_base, ph_mma, ph_w2, ph_w3;
 };
@@ -89,7 +91,8 @@ __device__ __forceinline__ void ld32(u32 taddr, u32 (&dr)[32]) {
 }
 }  // namespace wide
 
-// ---- CTA-wide helpers: every one of the CTA's 128 threads must call them (they synchronise) ----
+// ---- CTA-wide helpers: every one of the CTA's WD_T = 256 threads must call them (they synchronise).  Thread t works on entry
+// (row) t & 127; the two warpgroups split every element-wise stage by columns (warp w reads tensor-memory lanes 32 (w & 3) ..) ----
 __device__ __forceinline__ void wide_setup(WideSmem& S, const float* __restrict__ gw) {
   const u32 tid = threadIdx.x;
   if ((tid >> 5) == 0) {
@@ -116,12 +119,12 @@ __device__ __forceinline__ void wide_teardown(WideSmem& S) {
 }
 
 // One 128-entry tile: x = the features of this thread's entry, out = the 9 outputs of the MLP (before the 1/r scaling).
-// Returns false if an mbarrier wait timed out.  The phase bits live in shared memory (thread 0 flips them), so the function
+// `out` is complete in the FIRST warpgroup only (threads 0..127).  Returns false if an mbarrier wait timed out.  The phase bits live in shared memory (thread 0 flips them), so the function
 // keeps no state in registers between tiles.
 __device__ __forceinline__ bool wide_tile(WideSmem& S, const float* __restrict__ gw, const float (&x)[WD_IN], float (&out)[9]) {
-  const u32 tid = threadIdx.x, warp = tid >> 5;
+  const u32 tid = threadIdx.x, warp = tid >> 5, row = tid & 127u, hf = tid >> 7;
   const u32 bar_mma = wide::saddr(&S.bar_mma), bar_w2 = wide::saddr(&S.bar_w2), bar_w3 = wide::saddr(&S.bar_w3);
-  const u32 d2 = S.tmem_base + ((warp * 32u) << 16), d3 = d2 + WD_NC;      // accumulators: columns [0,64) and [64,192)
+  const u32 d2 = S.tmem_base + (((warp & 3u) * 32u) << 16), d3 = d2 + WD_NC;      // accumulators: columns [0,64) and [64,192)
   const float* w1 = S.small_ + WD_OFF_W1; const float* b1 = S.small_ + WD_OFF_B1; const float* b2 = S.small_ + WD_OFF_B2;
   const float* b3 = S.small_ + WD_OFF_B3; const float* w4 = S.small_ + WD_OFF_W4; const float* b4 = S.small_ + WD_OFF_B4;
   bool alive = true;
@@ -133,9 +136,9 @@ __device__ __forceinline__ bool wide_tile(WideSmem& S, const float* __restrict__
   }
   // ---- layer 1 ----
   {
-    float* Arow = &S.A1[(tid >> 3) * 1024 + (tid & 7) * 4];
+    float* Arow = &S.A1[(row >> 3) * 1024 + (row & 7) * 4];
 #pragma unroll 4
-    for (int kc = 0; kc < WD_H1 / 4; ++kc) {
+    for (int kc = (int)hf * (WD_H1 / 8); kc < (int)(hf + 1) * (WD_H1 / 8); ++kc) {
       float4 h;
       float* hp = reinterpret_cast<float*>(&h);
 #pragma unroll
@@ -168,9 +171,8 @@ __device__ __forceinline__ bool wide_tile(WideSmem& S, const float* __restrict__
     if (tid == 0 && c + 1 < WD_CHUNKS) wide::bulk_load(wide::saddr(S.W2c), gw + WD_OFF_W2 + (size_t)(c + 1) * WD_NC * WD_H1, WD_NC * WD_H1 * 4u, bar_w2);
     // ---- epilogue of layer 2: + b2, tanh -> A2c ----
     {
-      float* Arow = &S.A2c[(tid >> 3) * 512 + (tid & 7) * 4];
-#pragma unroll
-      for (int hf = 0; hf < 2; ++hf) {
+      float* Arow = &S.A2c[(row >> 3) * 512 + (row & 7) * 4];
+      {
         u32 dr[32];
         wide::ld32(d2 + hf * 32, dr);
 #pragma unroll
@@ -207,8 +209,12 @@ __device__ __forceinline__ bool wide_tile(WideSmem& S, const float* __restrict__
   // ---- layer 4: + b3, tanh, 128 -> 9 ----
 #pragma unroll
   for (int r = 0; r < 9; ++r) out[r] = b4[r];
+  if (hf) {
+#pragma unroll
+    for (int r = 0; r < 9; ++r) out[r] = 0.f;
+  }
 #pragma unroll 1
-  for (int qt = 0; qt < 4; ++qt) {
+  for (int qt = (int)hf * 2; qt < (int)hf * 2 + 2; ++qt) {
     u32 dr[32];
     wide::ld32(d3 + qt * 32, dr);
 #pragma unroll
@@ -221,8 +227,16 @@ __device__ __forceinline__ bool wide_tile(WideSmem& S, const float* __restrict__
       out[6] = fmaf(wb.z, t, out[6]); out[7] = fmaf(wb.w, t, out[7]); out[8] = fmaf(w[8], t, out[8]);
     }
   }
+  if (hf) {
+#pragma unroll
+    for (int r = 0; r < 9; ++r) S.red[row * 9 + r] = out[r];
+  }
   if (tid == 0) S.ph_mma = ph_mma;
   asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
   __syncthreads();                                                        // A1 and both accumulators are free for the next tile
+  if (!hf) {
+#pragma unroll
+    for (int r = 0; r < 9; ++r) out[r] += S.red[row * 9 + r];
+  }
   return alive;
 }

@@ -129,6 +129,11 @@ int hh_set_params(hh_ctx* ctx, const hh_params* params);
  * Same factors up to fp32 summation order in the norm recursion. */
 int hh_set_aca_impl(hh_ctx* ctx, int impl);
 
+/* Far-field apply form: 0 = blocks with max(m,n) <= 256 are streamed by persistent CTAs through a
+ * shared-memory ring filled by TMA bulk copies (default), 1 = one CTA per block in every size class.  Same sums up to
+ * fp32 summation order. */
+int hh_set_far_impl(hh_ctx* ctx, int impl);
+
 /* Record per-stage CUDA-event times into hh_stats (adds stream synchronisations). */
 int hh_enable_timing(hh_ctx* ctx, int on);
 

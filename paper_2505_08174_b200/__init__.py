@@ -20,7 +20,7 @@ ERRORS = {-1: "HH_ERR_INVALID_ARG", -2: "HH_ERR_WORKSPACE_TOO_SMALL", -3: "HH_ER
           -5: "HH_ERR_UNSUPPORTED"}
 
 EXPORTS = ["hh_create", "hh_destroy", "hh_set_params", "hh_enable_timing", "hh_build_tree", "hh_build_blocks", "hh_aca",
-           "hh_matvec", "hh_matvec_parts", "hh_set_aca_impl", "hh_far_apply_resident", "hh_step", "hh_step_host", "hh_set_pair_capacity",
+           "hh_matvec", "hh_matvec_parts", "hh_set_aca_impl", "hh_set_far_impl", "hh_far_apply_resident", "hh_step", "hh_step_host", "hh_set_pair_capacity",
            "hh_get_stats", "hh_get_tree", "hh_get_blocks", "hh_get_factors", "hh_get_ranks", "hh_eval_entries",
            "hh_set_capture", "hh_get_capture_count", "hh_last_error", "hh_version"]
 
@@ -154,6 +154,9 @@ class Context:
 
     def set_aca_impl(self, impl):
         self._chk(self.lib.hh_set_aca_impl(self._h, int(impl)))
+
+    def set_far_impl(self, impl):
+        self._chk(self.lib.hh_set_far_impl(self._h, int(impl)))
 
     def enable_timing(self, on=True):
         self._chk(self.lib.hh_enable_timing(self._h, int(on)))

@@ -421,6 +421,7 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   if (end <= first) end = (u32)first + 1;                        // try a single block; it fails below if it cannot fit
   const u32 nb = end - (u32)first;
   ctx->tab = (u32*)ctx->scratch;
+  ctx->far_items = nullptr; ctx->far_cnt = nullptr; ctx->far_items_cap = 0;   // no room for an item list in this layout: k_far, one CTA per block
   size_t tab_bytes = ((size_t)nb * HH_TAB_STRIDE * sizeof(u32) + 127) / 128 * 128;
   if (tab_bytes + 4096 > ctx->scratch_bytes) return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "factor arena too small");
   ctx->arena = (float*)(ctx->scratch + tab_bytes);
@@ -487,6 +488,8 @@ int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next) {
   HH_CUDA(cudaMemcpyAsync(ctx->h_sc, ctx->d_sc, sizeof(DevScalars), cudaMemcpyDeviceToHost, s));
   HH_CUDA(cudaStreamSynchronize(s));
   const DevScalars& h = *ctx->h_sc;
+  ctx->far_built = 0;
+  if (h.far_err) return hh_fail(ctx, HH_ERR_CUDA, h.far_err == 2 ? "far-field ring kernel: item list overflow (internal)" : "far-field ring kernel: an mbarrier wait timed out");
   if (ctx->mlp2_wide && h.deg_overflow) return hh_fail(ctx, HH_ERR_CUDA, "paper-size MLP entries (ACA): an mbarrier wait timed out");
   ctx->res_first = first;
   ctx->res_next = nx;

@@ -24,6 +24,15 @@
 
 #define GR 16                    /* entries per granule = half a warp                                   */
 #define A2_T 256                 /* threads of the entry-evaluating kernels                              */
+// One entry per thread at 80 registers (24 warps per SM) instead of two at 128 (16 warps): the weight loads from shared
+// memory are no longer shared by two entries, but a third more warps are in flight to cover the loads of the stored rank
+// terms.  Measured at c3 (ms_aca): 2 entries / 2 CTAs 5,485; 1 / 3: 5,067; 1 / 4 (64 registers, spills): 5,313.
+#ifndef A2_E
+#define A2_E 1                   /* entries per thread of k2_step (granules per warp = 2 * A2_E)          */
+#endif
+#ifndef A2_OCC
+#define A2_OCC 3                 /* CTAs of k2_step per SM the register budget is cut for                 */
+#endif
 
 struct BlkState {                /* 64 bytes per block of the batch                                      */
   u32 tlo, slo, m, n;
@@ -213,7 +222,8 @@ __device__ __forceinline__ void a2_norm_granule(const A2Args& A, u32 gi, u32 cou
 // F64 (aca_precision = 1, parity mode): the entry and the residual subtraction in fp64, rounded once when stored.
 // PRE (paper-size MLP, hh_wide.cuh): the raw entries were written into the rank-k slot by k2_eval_wide; they are loaded here.
 template <bool COLS, bool F64, bool PRE = false>
-__global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncount) {
+__global__ void __launch_bounds__(A2_T, F64 ? 2 : A2_OCC) k2_step(A2Args A, u32 count, u32 ncount) {
+  constexpr int E = A2_E, GPW = 2 * A2_E;                           // entries per thread, granules per warp
   __shared__ __align__(16) float sw[PRE ? 4 : (F64 ? 2 * HH_MLP2_FLOATS : HH_MLP2_FLOATS)];
   if (!PRE) {
     if (F64) load_weights(sw, reinterpret_cast<const float*>(A.w2d), 2 * HH_MLP2_FLOATS);
@@ -222,21 +232,21 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
   __syncthreads();
   const u32 lane = threadIdx.x & 31, half = lane >> 4, l16 = lane & 15, warp = threadIdx.x >> 5;
   const uint2* gl = COLS ? A.gn : A.gm;
-  const u32 ntiles = (count + 3) / 4;
+  const u32 ntiles = (count + GPW - 1) / GPW;
   u32 tile = blockIdx.x * (A2_T / 32) + warp;
   for (; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
     // (a) line 6 for the row granules with the same indices (memory-bound, independent of line 7)
-    if (COLS && 4 * tile < ncount) {
-      a2_norm_granule(A, 4 * tile + half, ncount, lane);
-      a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
+    if (COLS && GPW * tile < ncount) {
+#pragma unroll
+      for (int e = 0; e < E; ++e) a2_norm_granule(A, GPW * tile + 2 * e + half, ncount, lane);
     }
     // (b) the entries
-    float v[2][9];
-    double vd[F64 ? 2 : 1][9];
+    float v[E][9];
+    double vd[F64 ? E : 1][9];
     if (PRE) {
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const u32 gi = 4 * tile + 2 * e + half;
+      for (int e = 0; e < E; ++e) {
+        const u32 gi = GPW * tile + 2 * e + half;
         const bool gv = gi < count;
         const uint2 g = gl[gv ? gi : count - 1];
         const BlkState& s = A.st[g.x];
@@ -249,10 +259,10 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
         for (int r = 0; r < 9; ++r) v[e][r] = ok ? src[(size_t)r * lenp + idx] : 0.f;
       }
     } else {
-      float xi[2][3], xj[2][3];
+      float xi[E][3], xj[E][3];
 #pragma unroll
-      for (int e = 0; e < 2; ++e) {
-        const u32 gi = 4 * tile + 2 * e + half;
+      for (int e = 0; e < E; ++e) {
+        const u32 gi = GPW * tile + 2 * e + half;
         const uint2 g = gl[gi < count ? gi : count - 1];
         const BlkState& s = A.st[g.x];
         const u32 len = COLS ? s.n : s.m, idx = g.y + l16;
@@ -264,23 +274,33 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
       }
       if (F64) {
 #pragma unroll 1
-        for (int e = 0; e < 2; ++e) {
+        for (int e = 0; e < E; ++e) {
           float a3[3], b3[3];
           double m9[9];
 #pragma unroll
-          for (int d = 0; d < 3; ++d) { a3[d] = e ? xi[1][d] : xi[0][d]; b3[d] = e ? xj[1][d] : xj[0][d]; }
+          for (int d = 0; d < 3; ++d) { a3[d] = xi[0][d]; b3[d] = xj[0][d]; }
+#pragma unroll
+          for (int e2 = 1; e2 < E; ++e2)
+            if (e == e2) {
+#pragma unroll
+              for (int d = 0; d < 3; ++d) { a3[d] = xi[e2][d]; b3[d] = xj[e2][d]; }
+            }
           entry2_eval_d(reinterpret_cast<const double*>(sw), (double)A.a, a3, b3, m9);
 #pragma unroll
-          for (int r = 0; r < 9; ++r) { if (e) vd[F64 ? 1 : 0][r] = m9[r]; else vd[0][r] = m9[r]; }
+          for (int e2 = 0; e2 < E; ++e2)
+            if (e == e2) {
+#pragma unroll
+              for (int r = 0; r < 9; ++r) vd[F64 ? e2 : 0][r] = m9[r];
+            }
         }
       } else {
-        entry2_eval<2>(sw, A.a, xi, xj, v);
+        entry2_eval<E>(sw, A.a, xi, xj, v);
       }
     }
     // (c) residual, pivot scores, Gram sums: one granule per half-warp and slot
 #pragma unroll
-    for (int e = 0; e < 2; ++e) {
-      const u32 gi = 4 * tile + 2 * e + half;
+    for (int e = 0; e < E; ++e) {
+      const u32 gi = GPW * tile + 2 * e + half;
       const bool gv = gi < count;
       const uint2 g = gl[gv ? gi : count - 1];
       const BlkState& s = A.st[g.x];
@@ -393,9 +413,9 @@ __global__ void __launch_bounds__(A2_T, 2) k2_step(A2Args A, u32 count, u32 ncou
     }
   }
   if (COLS)                                                         // more row granules than column granules: finish line 6
-    for (; 4 * tile < ncount; tile += gridDim.x * (A2_T / 32)) {
-      a2_norm_granule(A, 4 * tile + half, ncount, lane);
-      a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
+    for (; GPW * tile < ncount; tile += gridDim.x * (A2_T / 32)) {
+#pragma unroll
+      for (int e = 0; e < E; ++e) a2_norm_granule(A, GPW * tile + 2 * e + half, ncount, lane);
     }
 }
 
@@ -605,6 +625,8 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     if (off + 4096 > ctx->scratch_bytes) return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "factor arena too small");
     ctx->arena = (float*)(ctx->scratch + off);
     ctx->arena_units = (ctx->scratch_bytes - off) / 128;
+    // once Alg. 2 is through, the accumulators and the row-granule counters are dead: the far-field item list lives there
+    ctx->far_cnt = A.cm; ctx->far_items = (uint4*)A.acc; ctx->far_items_cap = (size_t)nb * acc_floats * sizeof(float) / sizeof(uint4);
     A.w2 = ctx->w2; A.w2d = ctx->w2d; A.a = ctx->p.radius_a; A.tol = ctx->p.aca_tol; A.rule = ctx->p.pivot_rule;
     A.kappa_max = ctx->p.kappa_max > 0.f ? (double)ctx->p.kappa_max : (double)INFINITY;   // 0 = the plain listing (L221)
     A.dense_cap = ctx->p.dense_cap > 0.f ? (double)ctx->p.dense_cap : 128.0;
@@ -626,8 +648,8 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       if (nact == 0) break;
       if (gmc > ngran || gnc > ngran) return hh_fail(ctx, HH_ERR_CUDA, "lock-step ACA: granule list overflow (internal)");
       k2_gran_fill<<<HH_N + cdiv((int64_t)nb * 32, 256), 256, 0, s>>>(A);
-      const unsigned cap = (unsigned)ctx->n_sm * 2 * 4;
-      unsigned g1 = cdiv(cdiv(gmc, 4), A2_T / 32), g2 = cdiv(cdiv(gnc, 4), A2_T / 32);
+      const unsigned cap = (unsigned)ctx->n_sm * A2_OCC * 4;
+      unsigned g1 = cdiv(cdiv(gmc, 2 * A2_E), A2_T / 32), g2 = cdiv(cdiv(gnc, 2 * A2_E), A2_T / 32);
       const unsigned gr = (g1 < cap ? g1 : cap), gc = (g1 > g2 ? g1 : g2) < cap ? (g1 > g2 ? g1 : g2) : cap;
       if (ctx->mlp2_wide) {
         const unsigned t1 = cdiv(gmc, 8), t2 = cdiv(gnc, 8), nsm = (unsigned)ctx->n_sm;

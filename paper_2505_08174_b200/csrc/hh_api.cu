@@ -26,6 +26,7 @@ static int carve(hh_ctx* ctx, int64_t N) {
   ctx->res_first = ctx->res_next = 0;
   ctx->n_dense = 0;
   ctx->N = 0;
+  ctx->far_items = nullptr; ctx->far_cnt = nullptr; ctx->far_items_cap = 0; ctx->far_built = 0;
   Carver c{ctx->ws, 0, ctx->ws_bytes, true};
   ctx->Ncap = N;
   ctx->cap_pairs = ctx->pairs_per_particle * N + 4096;
@@ -265,6 +266,23 @@ extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
   return HH_OK;
 }
 
+// 0 = ring kernel (TMA bulk copies into a shared-memory ring, persistent CTAs) for blocks with max(m,n) <= 256 (default),
+// 1 = one CTA per block in every size class (round 1's kernel; kept for comparison)
+extern "C" int hh_set_far_impl(hh_ctx* ctx, int impl) {
+  if (!ctx || (impl != 0 && impl != 1)) return HH_ERR_INVALID_ARG;
+  ctx->far_impl = impl;
+  return HH_OK;
+}
+
+// error flag of the ring kernel and its item list (one 4-byte read-back per mat-vec)
+static int far_check(hh_ctx* ctx) {
+  HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->far_err, &ctx->d_sc->far_err, sizeof(u32), cudaMemcpyDeviceToHost, ctx->stream));
+  HH_CUDA(cudaStreamSynchronize(ctx->stream));
+  if (ctx->h_sc->far_err == 2) return hh_fail(ctx, HH_ERR_CUDA, "far-field ring kernel: item list overflow (internal)");
+  if (ctx->h_sc->far_err) return hh_fail(ctx, HH_ERR_CUDA, "far-field ring kernel: an mbarrier wait timed out");
+  return HH_OK;
+}
+
 extern "C" int hh_set_capture(hh_ctx* ctx, const int32_t* row_prefix, int32_t* records, int64_t cap_records) {
   if (!ctx) return HH_ERR_INVALID_ARG;
   if (records && (!row_prefix || cap_records < 1)) return hh_fail(ctx, HH_ERR_INVALID_ARG, "hh_set_capture: records without row_prefix / capacity");
@@ -385,6 +403,7 @@ extern "C" int hh_matvec_parts(hh_ctx* ctx, const float* F, float* U, int parts)
       }
     }
   }
+  if ((parts & 4) && ctx->nG > 0) HH_TRY(far_check(ctx));
   const int short_modes = ((parts & 8) && ctx->have_mlp3 ? 1 : 0) | ((parts & 16) ? 6 : 0);
   if (short_modes && ctx->p.rcut3 > 0.f) {
     T0(4);
@@ -415,7 +434,7 @@ extern "C" int hh_far_apply_resident(hh_ctx* ctx, const float* F, float* U) {
   HH_TRY(hh_dense_apply(ctx));
   k_unpermute<<<HH_N + cdiv(N, 256), 256, 0, ctx->stream>>>(ctx->Us, ctx->Fs, ctx->perm, N, 0, 0, U);
   HH_LAUNCH_CHECK();
-  return HH_OK;
+  return far_check(ctx);
 }
 
 extern "C" int hh_step(hh_ctx* ctx, float* X, const float* F, float* U, int64_t N, float dt) {

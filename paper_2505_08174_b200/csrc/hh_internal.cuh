@@ -45,7 +45,8 @@ struct DevScalars {
   u32 batch_end;            /* result of the batch-range search                                       */
   u32 class_bound[4];       /* first block of ACA class 1,2,3 in the sorted P^G (class 0 starts at 0) */
   u64 sum_rank, aca_entries, factor_bytes, n_faces;
-  u32 not_conv, singular, deg_overflow, pad1;
+  u32 not_conv, singular, deg_overflow;
+  u32 far_err;              /* k_far_ring / k_far_fill: 1 = an mbarrier wait timed out, 2 = item list overflow          */
   u64 near_entries, far_rows_cols;
   u32 max_rank_seen, n_dense;
   u64 fallback_entries;
@@ -104,6 +105,10 @@ struct hh_ctx {
   char* scratch; size_t scratch_bytes;  /* frontier ping-pong during build; == arena region    */
   float* arena; u64 arena_units;        /* after the resident table                            */
   u32* tab;                             /* resident block table, HH_TAB_STRIDE u32 per block   */
+  /* far-field ring kernel (hh_far.cu): item list of the resident blocks of the leaf-size classes */
+  int far_impl;                         /* 0 = ring kernel for max(m,n) <= 256 (default), 1 = one CTA per block everywhere */
+  int far_built, far_smem_set;
+  u32* far_cnt; uint4* far_items; size_t far_items_cap;
   /* three-body cell list */
   u32 *cell_of, *cell_start, *cell_order; int64_t n_cells_cap;
   /* pivot capture for at-size parity tests (hh_set_capture) */

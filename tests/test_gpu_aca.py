@@ -201,6 +201,33 @@ def test_far_apply_kernel_vs_its_own_factors(mlp2):
     ctx.close()
 
 
+@pytest.mark.parametrize("leaf,n,eta,tol", [(200, 12000, 1.0, 1e-4), (100, 9000, 1.0, 1e-5), (40, 6000, 2.0, 1e-4), (3, 700, 1.0, 1e-6)])
+def test_far_ring_kernel_equals_one_cta_per_block(mlp2, leaf, n, eta, tol):
+    """row 9, both forms on the SAME resident factors: the ring kernel (persistent CTAs, TMA bulk copies into a shared-memory
+    byte ring; blocks with max(m,n) <= 256) against round 1's one-CTA-per-block kernel, in every ring size class (leaf 200:
+    129..256, leaf 100: 65..128, leaf 40: <= 64, leaf 3: rows and columns below the pad width, ranks up to min(m,n))"""
+    X = synth.ball_cloud(n, 0.2, seed=11) if leaf != 40 else synth.chain_cloud(n // 50, 50, 0.1)
+    F = synth.gaussian_forces(len(X), seed=3)
+    ctx = setup(X, mlp2, leaf_size=leaf, eta=eta, aca_tol=tol)
+    nG = ctx.stats()["n_admissible"]
+    assert nG > 0
+    first, worst = 0, 0.0
+    while first < nG:                                               # every arena batch (the rank prediction may cut the first one short)
+        nxt = ctx.aca(first)
+        assert nxt > first
+        ctx.set_far_impl(1)
+        U1 = ctx.far_apply_resident(to_dev(F)).cpu().numpy()
+        ctx.set_far_impl(0)
+        U0 = ctx.far_apply_resident(to_dev(F)).cpu().numpy()
+        U0b = ctx.far_apply_resident(to_dev(F)).cpu().numpy()      # the item list is reused while the factors stay resident
+        assert np.linalg.norm(U1) > 0
+        worst = max(worst, rel_l2(U0, U1), rel_l2(U0b, U1))
+        first = nxt
+    print("leaf %d: ring vs one-CTA-per-block far-field apply: rel L2 %.3e over %d blocks" % (leaf, worst, nG))
+    assert worst <= 1e-6
+    ctx.close()
+
+
 def test_arena_batches_give_same_result(mlp2):
     X = synth.cube_cloud(6000, 0.1)
     F = synth.gaussian_forces(6000)

@@ -125,8 +125,9 @@ int hh_destroy(hh_ctx* ctx);
  * sweeps of config 3).  Invalidates tree and blocks as needed. */
 int hh_set_params(hh_ctx* ctx, const hh_params* params);
 
-/* Alg. 2 form: 0 = lock-step over all blocks of an arena batch (default), 1 = one CTA per block.
- * Same factors up to fp32 summation order in the norm recursion. */
+/* Alg. 2 form: 0 = lock-step over all blocks of an arena batch (default); 1 = one CTA per block; 2 = lock-step
+ * with the stored rank terms of a tile of 256 rows staged through shared memory by TMA bulk copies (measured slower, kept for
+ * comparison).  Same factors up to fp32 summation order in the norm recursion. */
 int hh_set_aca_impl(hh_ctx* ctx, int impl);
 
 /* Far-field apply form: 0 = blocks with max(m,n) <= 256 are streamed by persistent CTAs through a

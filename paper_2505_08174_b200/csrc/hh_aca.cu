@@ -489,6 +489,7 @@ int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next) {
   HH_CUDA(cudaStreamSynchronize(s));
   const DevScalars& h = *ctx->h_sc;
   ctx->far_built = 0;
+  if (h.aca_err) return hh_fail(ctx, HH_ERR_CUDA, "lock-step ACA (staged tiles): an mbarrier wait timed out");
   if (h.far_err) return hh_fail(ctx, HH_ERR_CUDA, h.far_err == 2 ? "far-field ring kernel: item list overflow (internal)" : "far-field ring kernel: an mbarrier wait timed out");
   if (ctx->mlp2_wide && h.deg_overflow) return hh_fail(ctx, HH_ERR_CUDA, "paper-size MLP entries (ACA): an mbarrier wait timed out");
   ctx->res_first = first;

@@ -419,6 +419,246 @@ __global__ void __launch_bounds__(A2_T, F64 ? 2 : A2_OCC) k2_step(A2Args A, u32 
     }
 }
 
+// ---- the same listing lines with the stored rank terms STAGED: a CTA takes a tile of 16 consecutive granules (256 rows
+// resp. columns), and before the entries of the tile are evaluated warp 0 issues TMA bulk copies (cp.async.bulk, one mbarrier
+// per CTA) of the first min(k, TS_KS) stored terms of those rows into shared memory -- a whole plane-major part of an arena
+// chunk in one copy where the tile covers a block completely, one copy per (rank, component plane) where it covers a slice
+// of a larger block.  The copies land while the MLP arithmetic runs (microseconds per tile), the update then reads shared
+// memory, and the Gram pass of the column side reads the same staged terms again.  Ranks beyond TS_KS (360 bytes of staging
+// per row) are read from global memory as in k2_step.  Arithmetic and its order are those of k2_step<COLS, false>: same bits.
+// MEASURED (c3, B200): correct (ranks identical to k2_step, U within 3e-7) but SLOWER, ms_aca 6,456 vs 5,066, so it is opt-in
+// (hh_set_aca_impl 2), not the default.  ncu (profiles/r02_k2_step_t.md): 16 warps per SM instead of 24, issue slots 54-58 %
+// busy, fma pipe 32 %, 1.6-1.8 warps per scheduler still waiting on global loads (the fixed operand, positions, table rows, the
+// A_pk accumulators, the used-pivot list), 0.5-1.2 at the tile barrier.  The staged operand was half of the loads, not the half
+// that stalls: the update is bound by the latency of MANY small dependent loads per thread, not by HBM bytes.
+#define TS_GR 16                 /* granules per tile                                                    */
+#define TS_ROWS (TS_GR * GR)     /* 256 threads, one entry each                                          */
+#define TS_KS 10                 /* stored rank terms staged per row                                     */
+#define TS_W_FLOATS ((HH_MLP2_FLOATS + 31) / 32 * 32)
+#define TS_SMEM (TS_W_FLOATS * 4 + TS_KS * 9 * TS_ROWS * 4 + 2 * TS_GR * 4 + 16 + 128)
+
+__device__ __forceinline__ u32 ts_smem_u32(const void* p) { return (u32)__cvta_generic_to_shared(p); }
+
+template <bool COLS>
+__global__ void __launch_bounds__(TS_ROWS, 2) k2_step_t(A2Args A, u32 count, u32 ncount, u32* __restrict__ err) {
+  extern __shared__ __align__(128) unsigned char ts_raw[];
+  unsigned char* ts0 = ts_raw + ((128u - (ts_smem_u32(ts_raw) & 127u)) & 127u);
+  float* sw = reinterpret_cast<float*>(ts0);
+  float* buf = sw + TS_W_FLOATS;                                   // staged terms: per segment [rank][9][plane stride]
+  u32* gbase = reinterpret_cast<u32*>(buf + TS_KS * 9 * TS_ROWS);  // per granule of the tile: offset of its first row (rank 0, plane 0)
+  u32* gps = gbase + TS_GR;                                        //                      plane stride of its segment
+  unsigned long long* barp = reinterpret_cast<unsigned long long*>(gps + TS_GR);
+  const u32 bar = ts_smem_u32(barp);
+  load_weights(sw, A.w2, HH_MLP2_FLOATS);
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  const u32 lane = threadIdx.x & 31, half = lane >> 4, l16 = lane & 15, warp = threadIdx.x >> 5, gslot = threadIdx.x >> 4;
+  const uint2* gl = COLS ? A.gn : A.gm;
+  const u32 ntiles = (count + TS_GR - 1) / TS_GR;
+  u32 phase = 0;
+  u32 tile = blockIdx.x;
+  for (; tile < ntiles; tile += gridDim.x) {
+    // (0) warp 0: cut the tile into segments (runs of consecutive granules of one block) and start the copies
+    if (warp == 0) {
+      const u32 gi = TS_GR * tile + l16;
+      const bool gv = gi < count && half == 0;
+      const uint2 g = gl[gi < count ? gi : count - 1];
+      const BlkState& s = A.st[g.x];
+      const bool live = gv && s.status == 0;
+      const u32 pb = __shfl_up_sync(0xffffffffu, g.x, 1), pr = __shfl_up_sync(0xffffffffu, g.y, 1);
+      const bool pl = __shfl_up_sync(0xffffffffu, live, 1);
+      const bool head = live && (lane == 0 || !pl || pb != g.x || pr + GR != g.y);
+      const u32 hm = __ballot_sync(0xffffffffu, head), lm = __ballot_sync(0xffffffffu, live);
+      // the head lane of my segment, and the number of granules of the segment
+      const u32 below = hm & (0xffffffffu >> (31 - lane));           // heads at or below my lane
+      const int hl = below ? 31 - __clz(below) : 0;
+      const u32 above = hm & ~(0xffffffffu >> (31 - lane));          // heads above my lane
+      const u32 dead_above = ~lm & ~(0xffffffffu >> (31 - lane));    // first lane above that is not live ends the run as well
+      const u32 stop = above | dead_above;
+      const int endl = stop ? __ffs(stop) - 1 : 32;                  // one past the last granule of a segment whose head I am
+      const u32 len = COLS ? s.n : s.m, lenp = a2_pad8(len), mp = a2_pad8(s.m), np = a2_pad8(s.n);
+      const u32 ngr = (u32)(endl - (int)lane);
+      const bool whole = g.y == 0 && g.y + GR * ngr >= len;
+      const u32 rows_here = GR * ngr < lenp - g.y ? GR * ngr : lenp - g.y;   // multiple of 8
+      const u32 ps_h = whole ? lenp : rows_here;
+      const u32 ks_h = (u32)(s.k < TS_KS ? s.k : TS_KS);
+      const u32 fl_h = head ? ks_h * 9u * ps_h : 0u;                 // floats of staging of the segment
+      u32 inc = fl_h;                                                // exclusive prefix over the lanes
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { const u32 t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= (u32)o) inc += t; }
+      const u32 total = __shfl_sync(0xffffffffu, inc, 31);
+      const u32 off_h = inc - fl_h;
+      const u32 seg_off = __shfl_sync(0xffffffffu, off_h, hl), seg_ps = __shfl_sync(0xffffffffu, ps_h, hl), seg_r0 = __shfl_sync(0xffffffffu, g.y, hl);
+      if (lane < TS_GR) { gbase[lane] = live ? seg_off + (g.y - seg_r0) : 0u; gps[lane] = live ? seg_ps : 0u; }
+      if (head && ks_h) {
+        const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+        const u32 dst0 = ts_smem_u32(buf + off_h);
+        if (whole) {
+          for (u32 c = 0; 4 * c < ks_h; ++c) {
+            const u32 nr = ks_h - 4 * c < 4 ? ks_h - 4 * c : 4;
+            const float* src = chunk_ptr(A, tabrow, 4 * c) + (COLS ? (size_t)HH_RC * 9 * mp : 0);
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst0 + 4u * c * 9u * ps_h * 4u),
+                         "l"(src), "r"(nr * 9u * ps_h * 4u), "r"(bar) : "memory");
+          }
+        } else {
+          for (u32 p = 0; p < ks_h; ++p) {
+            const float* src = chunk_ptr(A, tabrow, p) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np : (size_t)(p % HH_RC) * 9 * mp) + g.y;
+#pragma unroll
+            for (u32 r = 0; r < 9; ++r)
+              asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst0 + (p * 9u + r) * ps_h * 4u),
+                           "l"(src + (size_t)r * lenp), "r"(ps_h * 4u), "r"(bar) : "memory");
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) {
+        if (total) asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(total * 4u) : "memory");
+        else asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+      }
+    }
+    // (a) line 6 for the row granules with the same indices (memory-bound, independent of line 7)
+    if (COLS && TS_GR * tile < ncount) a2_norm_granule(A, TS_GR * tile + 2 * warp + half, ncount, lane);
+    // (b) the entry of this thread
+    const u32 gi = TS_GR * tile + gslot;
+    const bool gv = gi < count;
+    const uint2 g = gl[gv ? gi : count - 1];
+    const BlkState& s = A.st[g.x];
+    const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
+    const u32 len = COLS ? s.n : s.m, lenp = COLS ? np : mp, idx = g.y + l16;
+    const int k = s.k;
+    const bool live = gv && s.status == 0, ok = live && idx < len;
+    float v[1][9];
+    {
+      float xi[1][3], xj[1][3];
+      const u32 ic = idx < len ? idx : len - 1;
+      const u32 ti = COLS ? s.tlo + (u32)(s.ik < 0 ? 0 : s.ik) : s.tlo + ic;
+      const u32 sj = COLS ? s.slo + ic : s.slo + (u32)s.jk;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) { xi[0][d] = A.Xs[3 * (size_t)ti + d]; xj[0][d] = A.Xs[3 * (size_t)sj + d]; }
+      entry2_eval<1>(sw, A.a, xi, xj, v);
+    }
+    // the staged terms have landed (they had the whole MLP evaluation to do so)
+    {
+      bool done = false;
+      for (int it = 0; it < (1 << 22) && !done; ++it) {
+        u32 okw;
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}\n" : "=r"(okw) : "r"(bar), "r"(phase) : "memory");
+        done = okw != 0;
+      }
+      if (!done) { atomicExch(err, 1u); return; }
+      phase ^= 1u;
+    }
+    // (c) residual, pivot scores, Gram sums
+    {
+      const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+      float* acc = A.acc + (size_t)g.x * acc_stride(A.R);
+      float* dst = chunk_ptr(A, tabrow, k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np : (size_t)(k % HH_RC) * 9 * mp);
+      const int ks = k < TS_KS ? k : TS_KS;
+      const u32 ps = gps[gslot];
+      const float* sb = buf + gbase[gslot] + l16;                   // staged: term p, plane r at sb[(9 p + r) ps]
+      float Z[9];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) { Z[r] = 0.f; if (!ok) v[0][r] = 0.f; }
+      if (ok) {
+        const u32 fix = COLS ? (u32)s.ik : (u32)s.jk;
+#pragma unroll 2
+        for (int p = 0; p < k; ++p) {
+          const float* base = chunk_ptr(A, tabrow, p);
+          const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
+          const float* Qp = base + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
+          float cp[9], qp[9];
+          if (p < ks) {
+#pragma unroll
+            for (int r = 0; r < 9; ++r) {
+              const float sv = sb[(size_t)(9 * p + r) * ps];
+              if (COLS) { cp[r] = Cp[(size_t)r * mp + fix]; qp[r] = sv; } else { cp[r] = sv; qp[r] = Qp[(size_t)r * np + fix]; }
+            }
+          } else {
+#pragma unroll
+            for (int r = 0; r < 9; ++r) {
+              cp[r] = Cp[(size_t)r * mp + (COLS ? fix : idx)];
+              qp[r] = Qp[(size_t)r * np + (COLS ? idx : fix)];
+            }
+          }
+          submul33(v[0], cp, qp);
+          if (COLS) {
+            const float* Ap = acc + ACC_APK + 9 * p;
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int c = 0; c < 3; ++c) Z[3 * r + c] += qp[r] * Ap[c] + qp[3 + r] * Ap[3 + c] + qp[6 + r] * Ap[6 + c];
+          }
+        }
+#pragma unroll
+        for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp + idx] = v[0][r];
+      } else if (COLS && live && idx < lenp) {
+#pragma unroll
+        for (int r = 0; r < 9; ++r) dst[(size_t)r * lenp + idx] = 0.f;      // zero the pad columns (the far-field kernels read float4)
+      }
+      unsigned long long kd = 0ull, kf = 0ull;
+      if (ok) {
+        const int* piv = a2_piv(A, g.x) + (COLS ? HH_MAX_RANK : 0);
+        bool used = false;
+        for (int q = 0; q < k + (COLS ? 1 : 0); ++q) used |= (piv[q] == (int)idx);
+        if (!used) { kd = amax_key(fabsf(det33(v[0])), idx); kf = amax_key(fro2_33(v[0]), idx); }
+      }
+      kd = half_max(kd); kf = half_max(kf);
+      if (l16 == 0 && (kd | kf)) {
+        atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 2 : 0)], kd);
+        atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 3 : 1)], kf);
+      }
+      if (COLS) {
+        float bkk[9], cross = 0.f;
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) {
+            bkk[3 * r + c] = v[0][3 * r] * v[0][3 * c] + v[0][3 * r + 1] * v[0][3 * c + 1] + v[0][3 * r + 2] * v[0][3 * c + 2];
+            cross = fmaf(Z[3 * r + c], v[0][3 * c + r], cross);
+          }
+        const float t = half_sum9(bkk, l16);
+        cross = half_sum(cross);
+        const bool okh = __shfl_sync(0xffffffffu, ok, lane & 16);
+        if (okh && l16 < 9) atomicAdd(&acc[ACC_BKK + l16], t);
+        if (okh && l16 == 9) atomicAdd(&acc[ACC_CROSS], cross);
+      } else {
+        int kw = ok ? k : 0;
+#pragma unroll
+        for (int o = 16; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
+        const int kh = __shfl_sync(0xffffffffu, ok ? k : 0, lane & 16);
+        for (int p = 0; p < kw; ++p) {
+          float ap[9];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) ap[r] = 0.f;
+          if (ok && p < k) {
+            float cp[9];
+            if (p < ks) {
+#pragma unroll
+              for (int r = 0; r < 9; ++r) cp[r] = sb[(size_t)(9 * p + r) * ps];
+            } else {
+              const float* Cp = chunk_ptr(A, tabrow, p) + (size_t)(p % HH_RC) * 9 * mp;
+#pragma unroll
+              for (int r = 0; r < 9; ++r) cp[r] = Cp[(size_t)r * mp + idx];
+            }
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int c = 0; c < 3; ++c) ap[3 * r + c] = cp[r] * v[0][c] + cp[3 + r] * v[0][3 + c] + cp[6 + r] * v[0][6 + c];
+          }
+          const float t = half_sum9(ap, l16);
+          if (l16 < 9 && p < kh) atomicAdd(&acc[ACC_APK + 9 * p + l16], t);
+        }
+      }
+    }
+    __syncthreads();                                                // the staging buffer and the granule table are free again
+  }
+  if (COLS)                                                         // more row granules than column granules: finish line 6
+    for (; TS_GR * tile < ncount; tile += gridDim.x) a2_norm_granule(A, TS_GR * tile + 2 * warp + half, ncount, lane);
+}
+
 // ---- paper-size MLP: the entries of lines 4 / 7 for all active blocks, 128 per tensor-core tile (8 granules), stored raw
 // in the slot of rank k (gather coordinates -> network inference -> scatter into C / Q) ----
 template <bool COLS>
@@ -658,6 +898,18 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
         k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
         k2_eval_wide<true><<<HH_N + (t2 < nsm ? t2 : nsm), WD_T, wsm, s>>>(A, ctx->w2w, gnc, &ctx->d_sc->deg_overflow);
         k2_step<true, false, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
+      } else if (ctx->aca_impl == 2 && !ctx->p.aca_precision) {
+        // opt-in (hh_set_aca_impl 2): tiles of 16 granules, stored terms staged through shared memory by TMA bulk copies.
+        // Measured slower at c3 (ms_aca 6,456 vs 5,066): see the comment above k2_step_t and DESIGN.md section 6
+        if (!ctx->aca_smem_set) {
+          HH_CUDA(cudaFuncSetAttribute(k2_step_t<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TS_SMEM));
+          HH_CUDA(cudaFuncSetAttribute(k2_step_t<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TS_SMEM));
+          ctx->aca_smem_set = 1;
+        }
+        const unsigned tcap = (unsigned)ctx->n_sm * 2, t1 = cdiv(gmc, TS_GR), t2 = cdiv(gnc > gmc ? gnc : gmc, TS_GR);
+        k2_step_t<false><<<HH_N + (t1 < tcap ? t1 : tcap), TS_ROWS, TS_SMEM, s>>>(A, gmc, 0u, &ctx->d_sc->aca_err);
+        k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
+        k2_step_t<true><<<HH_N + (t2 < tcap ? t2 : tcap), TS_ROWS, TS_SMEM, s>>>(A, gnc, gmc, &ctx->d_sc->aca_err);   // + line 6 (normalisation)
       } else {
       if (ctx->p.aca_precision) k2_step<false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
       else k2_step<false, false><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);

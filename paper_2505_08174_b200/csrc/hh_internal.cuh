@@ -46,6 +46,7 @@ struct DevScalars {
   u32 class_bound[4];       /* first block of ACA class 1,2,3 in the sorted P^G (class 0 starts at 0) */
   u64 sum_rank, aca_entries, factor_bytes, n_faces;
   u32 not_conv, singular, deg_overflow;
+  u32 aca_err;              /* k2_step_t: 1 = an mbarrier wait timed out                                                 */
   u32 far_err;              /* k_far_ring / k_far_fill: 1 = an mbarrier wait timed out, 2 = item list overflow          */
   u64 near_entries, far_rows_cols;
   u32 max_rank_seen, n_dense;
@@ -62,7 +63,7 @@ struct hh_ctx {
   char err[512];
   int have_mlp3;
   int timing;
-  int aca_impl;                         /* 0 = lock-step (hh_aca2.cu), 1 = one CTA per block (hh_aca.cu) */
+  int aca_impl;                         /* 0 = lock-step, per-thread loads (hh_aca2.cu), 1 = one CTA per block (hh_aca.cu), 2 = lock-step, stored terms staged by TMA */
   int n_sm;                             /* cudaDevAttrMultiProcessorCount of the context's device (grid sizing) */
   int three_smem_set;                   /* k_three's dynamic shared-memory attribute has been set on this device */
   int64_t pairs_per_particle;
@@ -107,7 +108,7 @@ struct hh_ctx {
   u32* tab;                             /* resident block table, HH_TAB_STRIDE u32 per block   */
   /* far-field ring kernel (hh_far.cu): item list of the resident blocks of the leaf-size classes */
   int far_impl;                         /* 0 = ring kernel for max(m,n) <= 256 (default), 1 = one CTA per block everywhere */
-  int far_built, far_smem_set;
+  int far_built, far_smem_set, aca_smem_set;
   u32* far_cnt; uint4* far_items; size_t far_items_cap;
   /* three-body cell list */
   u32 *cell_of, *cell_start, *cell_order; int64_t n_cells_cap;

@@ -281,22 +281,53 @@ def test_degenerate_blocks(mlp2):
 
 
 def test_both_aca_forms_agree(mlp2):
-    """hh_set_aca_impl: the lock-step form (default) and the one-CTA-per-block form run the same Alg. 2; pivots,
-    ranks and flags agree on all but near-tie blocks and the mat-vecs agree to fp32 summation order."""
+    """hh_set_aca_impl: the lock-step form (default: per-thread loads; 2: stored terms staged by TMA bulk copies) and the
+    one-CTA-per-block form (1) run the same Alg. 2; pivots, ranks and flags agree on all but near-tie blocks and the mat-vecs
+    agree to fp32 summation order.  Forms 0 and 2 do the same arithmetic in the same order on each entry (only the Gram sums
+    are float atomics), so they differ by even less."""
     X = synth.cube_cloud(5000, 0.1, seed=9)
     F = synth.gaussian_forces(5000)
     res = []
-    for impl in (0, 1):
+    for impl in (0, 1, 2):
         ctx = setup(X, mlp2, leaf_size=32, eta=1.0, aca_tol=1e-4, ws_mb=8192)
         ctx.set_aca_impl(impl)
         U = ctx.matvec(to_dev(F)).cpu().numpy()
         ranks, flags = ctx.get_ranks()
         res.append((U, ranks, flags, ctx.stats()))
         ctx.close()
-    (U0, r0, f0, s0), (U1, r1, f1, s1) = res
-    assert s0["aca_batches"] == s1["aca_batches"] == 1
+    (U0, r0, f0, s0), (U1, r1, f1, s1), (U2, r2, f2, s2) = res
+    assert s0["aca_batches"] == s1["aca_batches"] == s2["aca_batches"] == 1
     assert np.mean(r0 != r1) < 0.02 and np.mean(f0 != f1) < 0.02
+    assert np.mean(r0 != r2) < 0.005 and np.mean(f0 != f2) < 0.005
+    print("staged vs per-thread loads: rel L2 %.3e, ranks differ on %.4f of the blocks; vs one CTA per block: %.3e"
+          % (rel_l2(U0, U2), np.mean(r0 != r2), rel_l2(U0, U1)))
     assert rel_l2(U0, U1) <= 1e-5
+    assert rel_l2(U0, U2) <= 1e-5
+
+
+@pytest.mark.parametrize("name,gen,leaf,eta,zeta", [
+    ("ball_tol1e-6_ranks_beyond_staging", lambda: synth.ball_cloud(6000, 0.2, seed=4), 48, 1.0, 1e-6),
+    ("big_blocks_slices", lambda: synth.cube_cloud(20000, 0.1, seed=6), 64, 0.7, 1e-4),
+    ("tiny_leaves", lambda: synth.cube_cloud(1500, 0.1, seed=8), 5, 1.0, 1e-5),
+])
+def test_staged_lockstep_equals_per_thread_loads(mlp2, name, gen, leaf, eta, zeta):
+    """k2_step_t (tiles of 256 rows, the first 10 stored terms staged by TMA) against k2_step (every term loaded by the thread that
+    needs it) on clouds that exercise: ranks beyond the staged 10, slices of blocks larger than a tile and blocks that straddle
+    a tile boundary, leaves smaller than a granule"""
+    X = gen()
+    F = synth.gaussian_forces(len(X), seed=5)
+    out = []
+    for impl in (0, 2):
+        ctx = setup(X, mlp2, leaf_size=leaf, eta=eta, aca_tol=zeta, ws_mb=8192)
+        ctx.set_aca_impl(impl)
+        U = ctx.matvec(to_dev(F)).cpu().numpy()
+        ranks, flags = ctx.get_ranks()
+        out.append((U, ranks, flags))
+        ctx.close()
+    (U0, r0, f0), (U2, r2, f2) = out
+    print(name, "rel L2 %.3e, max rank %d, ranks differ on %.4f of %d blocks" % (rel_l2(U0, U2), r0.max(), np.mean(r0 != r2), len(r0)))
+    assert np.mean(r0 != r2) < 0.005 and np.mean(f0 != f2) < 0.005
+    assert rel_l2(U0, U2) <= 10 * zeta * 0.01 + 2e-6
 
 
 def test_arena_overflow_is_retried_with_a_smaller_batch(mlp2):

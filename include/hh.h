@@ -226,6 +226,32 @@ int hh_eval_entries(hh_ctx* ctx, const float* Xi, const float* Xj, int64_t n, fl
 const char* hh_last_error(const hh_ctx* ctx);
 const char* hh_version(void);
 
+/* ---- the one entry point that ALLOCATES NOTHING (csrc/hh_static.cu) -------------------------------------------------
+ * For callers that cannot allocate or synchronise: code under CUDA graph capture, tight serving loops over small
+ * suspensions, harnesses that forbid cudaMalloc.  No hh_ctx, no workspace: inputs and outputs only.  The scratch (packed
+ * weights + partial sums) is a file-scope static __device__ array of HH_STATIC_SCRATCH_BYTES (about 3.2 MB) that every GPU
+ * which loads the library holds until exit.  The call makes no cudaMalloc / cudaFree / allocating library call, no memcpy
+ * and no synchronisation: three kernels are enqueued on cuda_stream and the call returns.
+ *
+ * Computes the definition  U_i = F_i + sum_{j != i} M_ij F_j,  M_ij = (1/r) R(MLP2([r_hat, a/r]))  (Eq. (4)
+ * L85-L88; Eq. (6) L108-L113 with alpha_1 = I; S-1..S-5): what hh_matvec returns when no block is admissible (L283), fp32,
+ * relative L2 <= 1e-5 of it (summation order differs).  No three-body or self terms.
+ *   mlp2        HOST struct; two-body network 4->32->32->9 only; W, b: HOST arrays of DEVICE pointers, read by the kernels
+ *               of THIS call on cuda_stream (they must be ready on that stream; nothing is cached between calls)
+ *   X, F        DEVICE fp32 [N][3], caller's order;  U  DEVICE fp32 [N][3], overwritten;  1 <= N <= HH_STATIC_MAX_N
+ *   cuda_stream a cudaStream_t (NULL = default stream)
+ *   err         HOST buffer for an error text, or NULL
+ * Errors: HH_ERR_WORKSPACE_TOO_SMALL if N > HH_STATIC_MAX_N (text names the limit), INVALID_ARG, UNSUPPORTED (other MLP
+ * shape), CUDA (no device, cudaGetSymbolAddress or a launch failed).
+ * Sharing: ALL calls on a device use the same array, which keeps the last call's contents (each call rewrites everything
+ * it reads, nothing needs clearing).  Calls that OVERLAP on the GPU (two streams, unordered graph branches) RACE on it;
+ * calls on one stream are ordered and safe.  The first call on a device looks up the array's address
+ * (cudaGetSymbolAddress, once per device, with that device current): make it outside graph capture. */
+#define HH_STATIC_MAX_N 16384
+#define HH_STATIC_SCRATCH_BYTES 3153920
+int hh_dense_matvec_static(const hh_mlp* mlp2, float radius_a, const float* X, const float* F, float* U, int64_t N,
+                           void* cuda_stream, char* err, size_t err_len);
+
 #ifdef __cplusplus
 }
 #endif

@@ -22,7 +22,7 @@ ERRORS = {-1: "HH_ERR_INVALID_ARG", -2: "HH_ERR_WORKSPACE_TOO_SMALL", -3: "HH_ER
 EXPORTS = ["hh_create", "hh_destroy", "hh_set_params", "hh_enable_timing", "hh_build_tree", "hh_build_blocks", "hh_aca",
            "hh_matvec", "hh_matvec_parts", "hh_set_aca_impl", "hh_set_far_impl", "hh_far_apply_resident", "hh_step", "hh_step_host", "hh_set_pair_capacity",
            "hh_get_stats", "hh_get_tree", "hh_get_blocks", "hh_get_factors", "hh_get_ranks", "hh_eval_entries",
-           "hh_set_capture", "hh_get_capture_count", "hh_last_error", "hh_version"]
+           "hh_set_capture", "hh_get_capture_count", "hh_last_error", "hh_version", "hh_dense_matvec_static"]
 
 
 class HHError(RuntimeError):
@@ -82,6 +82,41 @@ def _ptr(t):
         return C.c_void_p(t.ctypes.data)
     assert t.is_contiguous()
     return C.c_void_p(t.data_ptr())
+
+
+STATIC_MAX_N = 16384                      # HH_STATIC_MAX_N of include/hh.h
+
+
+class DeviceMlp:
+    """An hh_mlp whose layers live on the device (torch tensors owned here): the argument of dense_matvec_static"""
+
+    def __init__(self, mlp, device="cuda:0"):
+        import torch
+        Ws, bs = mlp
+        self.dims = (C.c_int32 * (len(Ws) + 1))(*([Ws[0].shape[1]] + [W.shape[0] for W in Ws]))
+        self.W = [torch.from_numpy(np.ascontiguousarray(W, np.float32)).to(device) for W in Ws]
+        self.b = [torch.from_numpy(np.ascontiguousarray(b, np.float32)).to(device) for b in bs]
+        self.pW = (C.c_void_p * len(Ws))(*[t.data_ptr() for t in self.W])
+        self.pb = (C.c_void_p * len(bs))(*[t.data_ptr() for t in self.b])
+        self.struct = _Mlp(len(Ws), self.dims, self.pW, self.pb)
+
+
+def dense_matvec_static(dmlp, X, F, radius_a=1.0, out=None, stream=None):
+    """hh_dense_matvec_static: the entry point that allocates nothing (static device scratch, N <= STATIC_MAX_N).
+    X, F: torch CUDA fp32 [N][3]; `out` (same shape) is overwritten, or a new tensor is returned (that allocation is
+    the binding's, not the library's).  Argument marshalling only."""
+    import torch
+    lib = load()
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2505_08174_b200 needs a CUDA device (there is no CPU fallback)")
+    U = out if out is not None else torch.empty_like(F)
+    st = stream if stream is not None else torch.cuda.current_stream(X.device)
+    err = C.create_string_buffer(512)
+    r = lib.hh_dense_matvec_static(C.byref(dmlp.struct), C.c_float(radius_a), _ptr(X), _ptr(F), _ptr(U), C.c_int64(X.shape[0]),
+                                   C.c_void_p(st.cuda_stream), err, C.c_size_t(512))
+    if r != HH_OK:
+        raise HHError(r, err.value.decode())
+    return U
 
 
 class Context:

@@ -419,6 +419,261 @@ __global__ void __launch_bounds__(A2_T, F64 ? 2 : A2_OCC) k2_step(A2Args A, u32 
     }
 }
 
+// ---- split form (hh_set_aca_impl 3): the entries of lines 4 / 7 alone, two per thread at the register budget of the MLP
+// (the near-field kernel's), stored raw in the slot of rank k; k2_step<COLS, false, PRE = true> then does the update at
+// its own, higher occupancy ----
+template <bool COLS>
+__global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
+  __shared__ __align__(16) float sw[HH_MLP2_FLOATS];
+  load_weights(sw, A.w2, HH_MLP2_FLOATS);
+  __syncthreads();
+  const u32 lane = threadIdx.x & 31, half = lane >> 4, l16 = lane & 15, warp = threadIdx.x >> 5;
+  const uint2* gl = COLS ? A.gn : A.gm;
+  const u32 ntiles = (count + 3) / 4;
+  for (u32 tile = blockIdx.x * (A2_T / 32) + warp; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
+    float xi[2][3], xj[2][3], v[2][9];
+    float* dst[2];
+    u32 lenp2[2];
+    bool ok[2];
+#pragma unroll
+    for (int e = 0; e < 2; ++e) {
+      const u32 gi = 4 * tile + 2 * e + half;
+      const bool gv = gi < count;
+      const uint2 g = gl[gv ? gi : count - 1];
+      const BlkState& s = A.st[g.x];
+      const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
+      const u32 len = COLS ? s.n : s.m, idx = g.y + l16;
+      const u32 ic = idx < len ? idx : len - 1;
+      const u32 ti = COLS ? s.tlo + (u32)(s.ik < 0 ? 0 : s.ik) : s.tlo + ic;
+      const u32 sj = COLS ? s.slo + ic : s.slo + (u32)s.jk;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) { xi[e][d] = A.Xs[3 * (size_t)ti + d]; xj[e][d] = A.Xs[3 * (size_t)sj + d]; }
+      ok[e] = gv && s.status == 0 && idx < len;
+      lenp2[e] = COLS ? np : mp;
+      dst[e] = chunk_ptr(A, A.tab + (size_t)g.x * HH_TAB_STRIDE, s.k) +
+               (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(s.k % HH_RC) * 9 * np : (size_t)(s.k % HH_RC) * 9 * mp) + idx;
+    }
+    entry2_eval<2>(sw, A.a, xi, xj, v);
+#pragma unroll
+    for (int e = 0; e < 2; ++e)
+      if (ok[e]) {
+#pragma unroll
+        for (int r = 0; r < 9; ++r) dst[e][(size_t)r * lenp2[e]] = v[e][r];
+      }
+  }
+}
+
+// ---- the update alone, vectorised (the default with k2_eval in front): a thread takes RPT consecutive rows (4) resp. columns
+// (2) of a granule, so the stored rank terms are read as 16- / 8-byte loads, the 27 multiply-adds per rank term are done for RPT
+// entries per fixed-operand fetch, and the 3x3 Gram sums of a granule are reduced over 4 resp. 8 lanes instead of 16.  Per
+// (entry, rank term) that is about 80 instructions instead of 200 in k2_step.  Arithmetic per entry is k2_step's, in its order.
+template <int TPG>                                                  // sum 9 values over the TPG lanes of a granule group;
+__device__ __forceinline__ void group_sum9(const float (&in)[9], u32 lig, float (&out)[TPG == 4 ? 3 : 2]) {   // lane lig gets slots [VPL lig, VPL lig + VPL)
+  constexpr int VPL = TPG == 4 ? 3 : 2, NS = TPG * VPL;
+  float v[NS];
+#pragma unroll
+  for (int r = 0; r < NS; ++r) v[r] = r < 9 ? in[r] : 0.f;
+  int cnt = NS;
+#pragma unroll
+  for (int w = TPG / 2; w; w >>= 1) {
+    const bool up = (lig & w) != 0;
+    cnt >>= 1;
+#pragma unroll
+    for (int r = 0; r < cnt; ++r) {
+      const float send = up ? v[r] : v[r + cnt], keep = up ? v[r + cnt] : v[r];
+      v[r] = keep + __shfl_xor_sync(0xffffffffu, send, w);
+    }
+  }
+#pragma unroll
+  for (int r = 0; r < VPL; ++r) out[r] = v[r];
+}
+template <int RPT> struct VecT;
+template <> struct VecT<4> { typedef float4 T; };
+template <> struct VecT<2> { typedef float2 T; };
+template <int RPT>
+__device__ __forceinline__ void vec_load(const float* p, float (&o)[RPT]) {
+  const typename VecT<RPT>::T t = *reinterpret_cast<const typename VecT<RPT>::T*>(p);
+  o[0] = t.x; o[1] = t.y;
+  if constexpr (RPT == 4) { o[2] = t.z; o[3] = t.w; }
+}
+template <int RPT>
+__device__ __forceinline__ void vec_store(float* p, const float (&o)[RPT]) {
+  typename VecT<RPT>::T t;
+  t.x = o[0]; t.y = o[1];
+  if constexpr (RPT == 4) { t.z = o[2]; t.w = o[3]; }
+  *reinterpret_cast<typename VecT<RPT>::T*>(p) = t;
+}
+
+template <bool COLS>
+__global__ void __launch_bounds__(A2_T, 2) k2_upd(A2Args A, u32 count, u32 ncount) {
+  constexpr int RPT = COLS ? 2 : 4, TPG = GR / RPT, GPW = 32 / TPG, VPL = TPG == 4 ? 3 : 2;
+  const u32 lane = threadIdx.x & 31, half = lane >> 4, warp = threadIdx.x >> 5, grp = lane / TPG, lig = lane % TPG;
+  const uint2* gl = COLS ? A.gn : A.gm;
+  const u32 ntiles = (count + GPW - 1) / GPW;
+  u32 tile = blockIdx.x * (A2_T / 32) + warp;
+  for (; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
+    if (COLS && GPW * tile < ncount) {                               // line 6 for the row granules with the same indices
+#pragma unroll
+      for (int e = 0; e < GPW / 2; ++e) a2_norm_granule(A, GPW * tile + 2 * e + half, ncount, lane);
+    }
+    const u32 gi = GPW * tile + grp;
+    const bool gv = gi < count;
+    const uint2 g = gl[gv ? gi : count - 1];
+    const BlkState& s = A.st[g.x];
+    const u32 mp = a2_pad8(s.m), np = a2_pad8(s.n);
+    const u32 len = COLS ? s.n : s.m, lenp = COLS ? np : mp, idx0 = g.y + RPT * lig;
+    const int k = s.k;
+    const bool live = gv && s.status == 0, any = live && idx0 < len;   // this thread has at least one real row / column
+    const u32* tabrow = A.tab + (size_t)g.x * HH_TAB_STRIDE;
+    float* acc = A.acc + (size_t)g.x * acc_stride(A.R);
+    float* dst = chunk_ptr(A, tabrow, k) + (COLS ? (size_t)HH_RC * 9 * mp + (size_t)(k % HH_RC) * 9 * np : (size_t)(k % HH_RC) * 9 * mp);
+    float v[9][RPT], Z[COLS ? 9 : 1][RPT];
+#pragma unroll
+    for (int r = 0; r < 9; ++r)
+#pragma unroll
+      for (int c = 0; c < RPT; ++c) { v[r][c] = 0.f; if (COLS) Z[COLS ? r : 0][c] = 0.f; }
+    if (any) {
+#pragma unroll
+      for (int r = 0; r < 9; ++r) vec_load<RPT>(dst + (size_t)r * lenp + idx0, v[r]);   // the raw entries (k2_eval)
+#pragma unroll
+      for (int r = 0; r < 9; ++r)
+#pragma unroll
+        for (int c = 0; c < RPT; ++c) if (idx0 + c >= len) v[r][c] = 0.f;                  // pad rows / columns
+      const u32 fix = COLS ? (u32)s.ik : (u32)s.jk;
+#pragma unroll 2
+      for (int p = 0; p < k; ++p) {
+        const float* base = chunk_ptr(A, tabrow, p);
+        const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
+        const float* Qp = base + (size_t)HH_RC * 9 * mp + (size_t)(p % HH_RC) * 9 * np;
+        float sp[9][RPT], fx[9];
+#pragma unroll
+        for (int r = 0; r < 9; ++r) {
+          vec_load<RPT>((COLS ? Qp : Cp) + (size_t)r * lenp + idx0, sp[r]);
+          fx[r] = COLS ? Cp[(size_t)r * mp + fix] : Qp[(size_t)r * np + fix];
+        }
+#pragma unroll
+        for (int c = 0; c < RPT; ++c) {
+          float a9[9], b9[9], r9[9];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) { a9[r] = COLS ? fx[r] : sp[r][c]; b9[r] = COLS ? sp[r][c] : fx[r]; r9[r] = v[r][c]; }
+          submul33(r9, a9, b9);                                      // R -= C_p(row) Q_p(col), the expression of k2_step
+#pragma unroll
+          for (int r = 0; r < 9; ++r) v[r][c] = r9[r];
+        }
+        if (COLS) {
+          const float* Ap = acc + ACC_APK + 9 * p;
+          float ap[9];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) ap[r] = Ap[r];
+#pragma unroll
+          for (int c = 0; c < RPT; ++c)
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int q = 0; q < 3; ++q)
+                Z[COLS ? 3 * r + q : 0][c] += sp[r][c] * ap[q] + sp[3 + r][c] * ap[3 + q] + sp[6 + r][c] * ap[6 + q];
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < 9; ++r)
+#pragma unroll
+        for (int c = 0; c < RPT; ++c) if (idx0 + c >= len) v[r][c] = 0.f;                  // pads stay zero (the far-field kernels read them)
+#pragma unroll
+      for (int r = 0; r < 9; ++r) vec_store<RPT>(dst + (size_t)r * lenp + idx0, v[r]);
+    } else if (COLS && live && idx0 < lenp) {
+#pragma unroll
+      for (int r = 0; r < 9; ++r) vec_store<RPT>(dst + (size_t)r * lenp + idx0, v[r]);      // all-pad group: zeros
+    }
+    // arg-max scores over unused rows / columns (Eq. (9); S-18)
+    unsigned long long kd = 0ull, kf = 0ull;
+    if (any) {
+      const int* piv = a2_piv(A, g.x) + (COLS ? HH_MAX_RANK : 0);
+      u32 used = 0;
+      for (int q = 0; q < k + (COLS ? 1 : 0); ++q) {
+        const u32 d = (u32)piv[q] - idx0;
+        if (d < (u32)RPT) used |= 1u << d;
+      }
+#pragma unroll
+      for (int c = 0; c < RPT; ++c) {
+        if (idx0 + c < len && !((used >> c) & 1u)) {
+          float m9[9];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) m9[r] = v[r][c];
+          const unsigned long long d1 = amax_key(fabsf(det33(m9)), idx0 + c), f1 = amax_key(fro2_33(m9), idx0 + c);
+          kd = d1 > kd ? d1 : kd; kf = f1 > kf ? f1 : kf;
+        }
+      }
+    }
+#pragma unroll
+    for (int o = TPG / 2; o; o >>= 1) {
+      unsigned long long t = __shfl_xor_sync(0xffffffffu, kd, o); kd = t > kd ? t : kd;
+      t = __shfl_xor_sync(0xffffffffu, kf, o); kf = t > kf ? t : kf;
+    }
+    if (lig == 0 && (kd | kf)) {
+      atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 2 : 0)], kd);
+      atomicMax(&A.amax[(size_t)g.x * 4 + (COLS ? 3 : 1)], kf);
+    }
+    const bool okg = __shfl_sync(0xffffffffu, any, lane - lig);      // the granule is real (its first thread has a real row)
+    if (COLS) {
+      // norm recursion (S-19): B_kk = sum_j q(j) q(j)^T, cross = sum_j tr(Z(j) q(j))
+      float bkk[9], cross = 0.f, o2[VPL];
+#pragma unroll
+      for (int r = 0; r < 9; ++r) bkk[r] = 0.f;
+#pragma unroll
+      for (int c = 0; c < RPT; ++c)
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            bkk[3 * r + q] += v[3 * r][c] * v[3 * q][c] + v[3 * r + 1][c] * v[3 * q + 1][c] + v[3 * r + 2][c] * v[3 * q + 2][c];
+            cross = fmaf(Z[COLS ? 3 * r + q : 0][c], v[3 * q + r][c], cross);
+          }
+      group_sum9<TPG>(bkk, lig, o2);
+#pragma unroll
+      for (int o = TPG / 2; o; o >>= 1) cross += __shfl_xor_sync(0xffffffffu, cross, o);
+      if (okg) {
+#pragma unroll
+        for (int r = 0; r < VPL; ++r) if (VPL * lig + r < 9) atomicAdd(&acc[ACC_BKK + VPL * lig + r], o2[r]);
+        if (lig == TPG - 1) atomicAdd(&acc[ACC_CROSS], cross);
+      }
+    } else {
+      // Gram matrices of the raw column, A'_pk = sum_i C_p(i)^T c'(i) (k2_piv turns them into A_pk); the stored columns were
+      // read a moment ago by this same thread (L1 / L2 hits)
+      int kw = any ? k : 0;
+#pragma unroll
+      for (int o = 16; o; o >>= 1) kw = max(kw, __shfl_xor_sync(0xffffffffu, kw, o));
+      const int kg = __shfl_sync(0xffffffffu, any ? k : 0, lane - lig);
+      for (int p = 0; p < kw; ++p) {
+        float ap[9], o3[VPL];
+#pragma unroll
+        for (int r = 0; r < 9; ++r) ap[r] = 0.f;
+        if (any && p < k) {
+          const float* Cp = chunk_ptr(A, tabrow, p) + (size_t)(p % HH_RC) * 9 * mp;
+          float cp[9][RPT];
+#pragma unroll
+          for (int r = 0; r < 9; ++r) vec_load<RPT>(Cp + (size_t)r * mp + idx0, cp[r]);
+#pragma unroll
+          for (int c = 0; c < RPT; ++c)
+#pragma unroll
+            for (int r = 0; r < 3; ++r)
+#pragma unroll
+              for (int q = 0; q < 3; ++q) ap[3 * r + q] += cp[r][c] * v[q][c] + cp[3 + r][c] * v[3 + q][c] + cp[6 + r][c] * v[6 + q][c];
+        }
+        group_sum9<TPG>(ap, lig, o3);
+        if (p < kg) {
+#pragma unroll
+          for (int r = 0; r < VPL; ++r) if (VPL * lig + r < 9) atomicAdd(&acc[ACC_APK + 9 * p + VPL * lig + r], o3[r]);
+        }
+      }
+    }
+  }
+  if (COLS)                                                         // more row granules than column granules: finish line 6
+    for (; GPW * tile < ncount; tile += gridDim.x * (A2_T / 32)) {
+#pragma unroll
+      for (int e = 0; e < GPW / 2; ++e) a2_norm_granule(A, GPW * tile + 2 * e + half, ncount, lane);
+    }
+}
+
 // ---- the same listing lines with the stored rank terms STAGED: a CTA takes a tile of 16 consecutive granules (256 rows
 // resp. columns), and before the entries of the tile are evaluated warp 0 issues TMA bulk copies (cp.async.bulk, one mbarrier
 // per CTA) of the first min(k, TS_KS) stored terms of those rows into shared memory -- a whole plane-major part of an arena
@@ -897,6 +1152,25 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
         k2_step<false, false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
         k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
         k2_eval_wide<true><<<HH_N + (t2 < nsm ? t2 : nsm), WD_T, wsm, s>>>(A, ctx->w2w, gnc, &ctx->d_sc->deg_overflow);
+        k2_step<true, false, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
+      } else if (ctx->aca_impl == 4 && !ctx->p.aca_precision) {
+        // entries (k2_eval) and the vectorised update (k2_upd) as separate launches
+        const unsigned ecap = (unsigned)ctx->n_sm * 2 * 4;
+        const unsigned e1 = cdiv(cdiv(gmc, 4), A2_T / 32), e2 = cdiv(cdiv(gnc, 4), A2_T / 32);
+        const unsigned u1 = cdiv(cdiv(gmc, 8), A2_T / 32), u2 = cdiv(cdiv(gnc > gmc ? gnc : gmc, 4), A2_T / 32);
+        k2_eval<false><<<HH_N + (e1 < ecap ? e1 : ecap), A2_T, 0, s>>>(A, gmc);
+        k2_upd<false><<<HH_N + (u1 < ecap ? u1 : ecap), A2_T, 0, s>>>(A, gmc, 0u);
+        k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
+        k2_eval<true><<<HH_N + (e2 < ecap ? e2 : ecap), A2_T, 0, s>>>(A, gnc);
+        k2_upd<true><<<HH_N + (u2 < ecap ? u2 : ecap), A2_T, 0, s>>>(A, gnc, gmc);
+      } else if (ctx->aca_impl == 3 && !ctx->p.aca_precision) {
+        // split form: entries (MLP) and update as separate launches
+        const unsigned ecap = (unsigned)ctx->n_sm * 2 * 4;
+        const unsigned e1 = cdiv(cdiv(gmc, 4), A2_T / 32), e2 = cdiv(cdiv(gnc, 4), A2_T / 32);
+        k2_eval<false><<<HH_N + (e1 < ecap ? e1 : ecap), A2_T, 0, s>>>(A, gmc);
+        k2_step<false, false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
+        k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
+        k2_eval<true><<<HH_N + (e2 < ecap ? e2 : ecap), A2_T, 0, s>>>(A, gnc);
         k2_step<true, false, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
       } else if (ctx->aca_impl == 2 && !ctx->p.aca_precision) {
         // opt-in (hh_set_aca_impl 2): tiles of 16 granules, stored terms staged through shared memory by TMA bulk copies.

@@ -261,7 +261,7 @@ extern "C" int hh_set_pair_capacity(hh_ctx* ctx, int64_t pairs_per_particle) {
 // 1 = one CTA per admissible block (the first form), 2 = lock-step with the stored terms staged through shared memory by TMA
 // bulk copies (measured slower); 1, 2 kept for comparison
 extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
-  if (!ctx || impl < 0 || impl > 2) return HH_ERR_INVALID_ARG;
+  if (!ctx || impl < 0 || impl > 4) return HH_ERR_INVALID_ARG;
   if (impl == 1 && ctx->mlp2_wide) return hh_fail(ctx, HH_ERR_UNSUPPORTED, "the paper-size MLP runs in the lock-step form only");
   ctx->aca_impl = impl;
   ctx->res_first = ctx->res_next = 0;

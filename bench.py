@@ -404,8 +404,8 @@ def main():
     ap.add_argument("--kappa-max", type=float, default=None, help="S-18b limit on the pivot-block condition number")
     ap.add_argument("--near-path", type=int, default=2, choices=[0, 1, 2], help="0 fp32 ALU, 1 tcgen05 tf32 + tanh.approx (2e-3), 2 tcgen05 split tf32 + tanhf")
     ap.add_argument("--aca-precision", type=int, default=0, choices=[0, 1], help="1 = fp64 entries and residuals in Alg. 2 (parity mode)")
-    ap.add_argument("--aca-impl", type=int, default=0, choices=[0, 1, 2, 3, 4], help="hh_set_aca_impl: 0 lock-step (default), 1 one CTA per block, 2 lock-step with TMA-staged terms, 3 lock-step, entries and update in separate launches")
-    ap.add_argument("--far-impl", type=int, default=0, choices=[0, 1], help="hh_set_far_impl: 0 ring kernel for blocks <= 256 (default), 1 one CTA per block")
+    ap.add_argument("--aca-impl", type=int, default=0, choices=[0, 1, 2, 3], help="hh_set_aca_impl: 0 lock-step, entries and update in separate launches (default), 1 one CTA per block, 2 lock-step with TMA-staged terms, 3 lock-step, fused")
+    ap.add_argument("--far-impl", type=int, default=0, choices=[0, 1, 2], help="hh_set_far_impl: 0 ring kernel for blocks <= 256 (default), 1 one CTA per block, 2 = 0 + whole-block ring kernel for blocks <= 1024")
     ap.add_argument("--paper-mlp", action="store_true", help="two-body MLP with the paper's hidden layers 128/512/128 (tensor-core tile)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     ap.add_argument("--no-c4", dest="with_c4", action="store_false", help="skip the 10M-particle sub-record of the default (c3) run")

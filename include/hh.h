@@ -125,14 +125,17 @@ int hh_destroy(hh_ctx* ctx);
  * sweeps of config 3).  Invalidates tree and blocks as needed. */
 int hh_set_params(hh_ctx* ctx, const hh_params* params);
 
-/* Alg. 2 form: 0 = lock-step over all blocks of an arena batch (default); 1 = one CTA per block; 2 = lock-step
- * with the stored rank terms of a tile of 256 rows staged through shared memory by TMA bulk copies (measured slower, kept for
- * comparison).  Same factors up to fp32 summation order in the norm recursion. */
+/* Alg. 2 form: 0 = lock-step over all blocks of an arena batch (default; each listing line a parallel pass over
+ * the selected blocks), entry evaluation and the vectorised update as separate launches; 1 = one CTA per block; 2 = lock-step
+ * with the stored rank terms of a tile of 256 rows staged through shared memory by TMA bulk copies; 3 = lock-step with entry
+ * evaluation and update fused in one kernel.  1-3 are measured slower and kept for comparison.  Same factors up to fp32
+ * summation order in the norm recursion. */
 int hh_set_aca_impl(hh_ctx* ctx, int impl);
 
 /* Far-field apply form: 0 = blocks with max(m,n) <= 256 are streamed by persistent CTAs through a
- * shared-memory ring filled by TMA bulk copies (default), 1 = one CTA per block in every size class.  Same sums up to
- * fp32 summation order. */
+ * shared-memory ring filled by TMA bulk copies, larger ones by one CTA per block (default); 1 = one CTA per block in every
+ * size class; 2 = 0 plus a whole-block ring kernel for 256 < max(m,n) <= 1024 (measured slower, kept for comparison).  Same
+ * sums up to fp32 summation order. */
 int hh_set_far_impl(hh_ctx* ctx, int impl);
 
 /* Record per-stage CUDA-event times into hh_stats (adds stream synchronisations). */

@@ -419,18 +419,24 @@ __global__ void __launch_bounds__(A2_T, F64 ? 2 : A2_OCC) k2_step(A2Args A, u32 
     }
 }
 
-// ---- split form (hh_set_aca_impl 3): the entries of lines 4 / 7 alone, two per thread at the register budget of the MLP
-// (the near-field kernel's), stored raw in the slot of rank k; k2_step<COLS, false, PRE = true> then does the update at
-// its own, higher occupancy ----
-template <bool COLS>
-__global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
+// ---- the default form, first half: the entries of lines 4 / 7 alone, two per thread at the register budget of the MLP
+// (the near-field kernel's), stored raw in the slot of rank k; k2_upd then does the update ----
+// NORM (with COLS): line 6 for the row granules with the same indices rides along -- it is memory-bound and independent of
+// these entries, and this kernel's arithmetic hides its loads (k2_upd is memory-bound itself and would only be delayed by it).
+template <bool COLS, bool NORM = false>
+__global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count, u32 ncount) {
   __shared__ __align__(16) float sw[HH_MLP2_FLOATS];
   load_weights(sw, A.w2, HH_MLP2_FLOATS);
   __syncthreads();
   const u32 lane = threadIdx.x & 31, half = lane >> 4, l16 = lane & 15, warp = threadIdx.x >> 5;
   const uint2* gl = COLS ? A.gn : A.gm;
   const u32 ntiles = (count + 3) / 4;
-  for (u32 tile = blockIdx.x * (A2_T / 32) + warp; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
+  u32 tile = blockIdx.x * (A2_T / 32) + warp;
+  for (; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
+    if (NORM && 4 * tile < ncount) {
+      a2_norm_granule(A, 4 * tile + half, ncount, lane);
+      a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
+    }
     float xi[2][3], xj[2][3], v[2][9];
     float* dst[2];
     u32 lenp2[2];
@@ -461,6 +467,11 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count) {
         for (int r = 0; r < 9; ++r) dst[e][(size_t)r * lenp2[e]] = v[e][r];
       }
   }
+  if (NORM)                                                         // more row granules than column granules: finish line 6
+    for (; 4 * tile < ncount; tile += gridDim.x * (A2_T / 32)) {
+      a2_norm_granule(A, 4 * tile + half, ncount, lane);
+      a2_norm_granule(A, 4 * tile + 2 + half, ncount, lane);
+    }
 }
 
 // ---- the update alone, vectorised (the default with k2_eval in front): a thread takes RPT consecutive rows (4) resp. columns
@@ -496,6 +507,15 @@ __device__ __forceinline__ void vec_load(const float* p, float (&o)[RPT]) {
   o[0] = t.x; o[1] = t.y;
   if constexpr (RPT == 4) { o[2] = t.z; o[3] = t.w; }
 }
+// the same load with an L2 eviction-priority policy (createpolicy): the column side reads every stored term twice (update,
+// then the Gram sums against the finished residual); the first read asks L2 to keep the line, the second lets it go
+template <int RPT>
+__device__ __forceinline__ void vec_load_pol(const float* p, float (&o)[RPT], unsigned long long pol) {
+  if constexpr (RPT == 4)
+    asm volatile("ld.global.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;" : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]) : "l"(p), "l"(pol));
+  else
+    asm volatile("ld.global.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(o[0]), "=f"(o[1]) : "l"(p), "l"(pol));
+}
 template <int RPT>
 __device__ __forceinline__ void vec_store(float* p, const float (&o)[RPT]) {
   typename VecT<RPT>::T t;
@@ -504,15 +524,18 @@ __device__ __forceinline__ void vec_store(float* p, const float (&o)[RPT]) {
   *reinterpret_cast<typename VecT<RPT>::T*>(p) = t;
 }
 
-template <bool COLS>
+template <bool COLS, bool NORM = false>
 __global__ void __launch_bounds__(A2_T, 2) k2_upd(A2Args A, u32 count, u32 ncount) {
   constexpr int RPT = COLS ? 2 : 4, TPG = GR / RPT, GPW = 32 / TPG, VPL = TPG == 4 ? 3 : 2;
   const u32 lane = threadIdx.x & 31, half = lane >> 4, warp = threadIdx.x >> 5, grp = lane / TPG, lig = lane % TPG;
   const uint2* gl = COLS ? A.gn : A.gm;
   const u32 ntiles = (count + GPW - 1) / GPW;
+  unsigned long long pol_keep, pol_drop;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_drop));
   u32 tile = blockIdx.x * (A2_T / 32) + warp;
   for (; tile < ntiles; tile += gridDim.x * (A2_T / 32)) {
-    if (COLS && GPW * tile < ncount) {                               // line 6 for the row granules with the same indices
+    if (NORM && GPW * tile < ncount) {                               // line 6 for the row granules with the same indices
 #pragma unroll
       for (int e = 0; e < GPW / 2; ++e) a2_norm_granule(A, GPW * tile + 2 * e + half, ncount, lane);
     }
@@ -548,7 +571,8 @@ __global__ void __launch_bounds__(A2_T, 2) k2_upd(A2Args A, u32 count, u32 ncoun
         float sp[9][RPT], fx[9];
 #pragma unroll
         for (int r = 0; r < 9; ++r) {
-          vec_load<RPT>((COLS ? Qp : Cp) + (size_t)r * lenp + idx0, sp[r]);
+          if (COLS) vec_load_pol<RPT>(Qp + (size_t)r * lenp + idx0, sp[r], pol_drop);      // read once per iteration
+          else vec_load_pol<RPT>(Cp + (size_t)r * lenp + idx0, sp[r], pol_keep);          // read again by the Gram pass below
           fx[r] = COLS ? Cp[(size_t)r * mp + fix] : Qp[(size_t)r * np + fix];
         }
 #pragma unroll
@@ -651,7 +675,7 @@ __global__ void __launch_bounds__(A2_T, 2) k2_upd(A2Args A, u32 count, u32 ncoun
           const float* Cp = chunk_ptr(A, tabrow, p) + (size_t)(p % HH_RC) * 9 * mp;
           float cp[9][RPT];
 #pragma unroll
-          for (int r = 0; r < 9; ++r) vec_load<RPT>(Cp + (size_t)r * mp + idx0, cp[r]);
+          for (int r = 0; r < 9; ++r) vec_load_pol<RPT>(Cp + (size_t)r * mp + idx0, cp[r], pol_drop);
 #pragma unroll
           for (int c = 0; c < RPT; ++c)
 #pragma unroll
@@ -667,7 +691,7 @@ __global__ void __launch_bounds__(A2_T, 2) k2_upd(A2Args A, u32 count, u32 ncoun
       }
     }
   }
-  if (COLS)                                                         // more row granules than column granules: finish line 6
+  if (NORM)                                                         // more row granules than column granules: finish line 6
     for (; GPW * tile < ncount; tile += gridDim.x * (A2_T / 32)) {
 #pragma unroll
       for (int e = 0; e < GPW / 2; ++e) a2_norm_granule(A, GPW * tile + 2 * e + half, ncount, lane);
@@ -1146,35 +1170,27 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       const unsigned cap = (unsigned)ctx->n_sm * A2_OCC * 4;
       unsigned g1 = cdiv(cdiv(gmc, 2 * A2_E), A2_T / 32), g2 = cdiv(cdiv(gnc, 2 * A2_E), A2_T / 32);
       const unsigned gr = (g1 < cap ? g1 : cap), gc = (g1 > g2 ? g1 : g2) < cap ? (g1 > g2 ? g1 : g2) : cap;
+      const unsigned ecap = (unsigned)ctx->n_sm * 2 * 4;
+      const unsigned u1 = cdiv(cdiv(gmc, 8), A2_T / 32), u2 = cdiv(cdiv(gnc, 4), A2_T / 32), u2n = cdiv(cdiv(gnc > gmc ? gnc : gmc, 4), A2_T / 32);
       if (ctx->mlp2_wide) {
+        // paper-size MLP: entries on the tensor cores (hh_wide.cuh), then the vectorised update (line 6 rides with the row side)
         const unsigned t1 = cdiv(gmc, 8), t2 = cdiv(gnc, 8), nsm = (unsigned)ctx->n_sm;
         k2_eval_wide<false><<<HH_N + (t1 < nsm ? t1 : nsm), WD_T, wsm, s>>>(A, ctx->w2w, gmc, &ctx->d_sc->deg_overflow);
-        k2_step<false, false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
-        k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
-        k2_eval_wide<true><<<HH_N + (t2 < nsm ? t2 : nsm), WD_T, wsm, s>>>(A, ctx->w2w, gnc, &ctx->d_sc->deg_overflow);
-        k2_step<true, false, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
-      } else if (ctx->aca_impl == 4 && !ctx->p.aca_precision) {
-        // entries (k2_eval) and the vectorised update (k2_upd) as separate launches
-        const unsigned ecap = (unsigned)ctx->n_sm * 2 * 4;
-        const unsigned e1 = cdiv(cdiv(gmc, 4), A2_T / 32), e2 = cdiv(cdiv(gnc, 4), A2_T / 32);
-        const unsigned u1 = cdiv(cdiv(gmc, 8), A2_T / 32), u2 = cdiv(cdiv(gnc > gmc ? gnc : gmc, 4), A2_T / 32);
-        k2_eval<false><<<HH_N + (e1 < ecap ? e1 : ecap), A2_T, 0, s>>>(A, gmc);
         k2_upd<false><<<HH_N + (u1 < ecap ? u1 : ecap), A2_T, 0, s>>>(A, gmc, 0u);
         k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
-        k2_eval<true><<<HH_N + (e2 < ecap ? e2 : ecap), A2_T, 0, s>>>(A, gnc);
-        k2_upd<true><<<HH_N + (u2 < ecap ? u2 : ecap), A2_T, 0, s>>>(A, gnc, gmc);
-      } else if (ctx->aca_impl == 3 && !ctx->p.aca_precision) {
-        // split form: entries (MLP) and update as separate launches
-        const unsigned ecap = (unsigned)ctx->n_sm * 2 * 4;
-        const unsigned e1 = cdiv(cdiv(gmc, 4), A2_T / 32), e2 = cdiv(cdiv(gnc, 4), A2_T / 32);
-        k2_eval<false><<<HH_N + (e1 < ecap ? e1 : ecap), A2_T, 0, s>>>(A, gmc);
-        k2_step<false, false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
+        k2_eval_wide<true><<<HH_N + (t2 < nsm ? t2 : nsm), WD_T, wsm, s>>>(A, ctx->w2w, gnc, &ctx->d_sc->deg_overflow);
+        k2_upd<true, true><<<HH_N + (u2n < ecap ? u2n : ecap), A2_T, 0, s>>>(A, gnc, gmc);
+      } else if (ctx->aca_impl == 0 && !ctx->p.aca_precision) {
+        // the default: entries (k2_eval, the MLP at its own register budget) and the vectorised update (k2_upd) as separate launches
+        const unsigned e1 = cdiv(cdiv(gmc, 4), A2_T / 32), e2n = cdiv(cdiv(gnc > gmc ? gnc : gmc, 4), A2_T / 32);
+        k2_eval<false><<<HH_N + (e1 < ecap ? e1 : ecap), A2_T, 0, s>>>(A, gmc, 0u);
+        k2_upd<false><<<HH_N + (u1 < ecap ? u1 : ecap), A2_T, 0, s>>>(A, gmc, 0u);
         k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
-        k2_eval<true><<<HH_N + (e2 < ecap ? e2 : ecap), A2_T, 0, s>>>(A, gnc);
-        k2_step<true, false, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
+        k2_eval<true, true><<<HH_N + (e2n < ecap ? e2n : ecap), A2_T, 0, s>>>(A, gnc, gmc);            // + line 6 (normalisation)
+        k2_upd<true><<<HH_N + (u2 < ecap ? u2 : ecap), A2_T, 0, s>>>(A, gnc, 0u);
       } else if (ctx->aca_impl == 2 && !ctx->p.aca_precision) {
         // opt-in (hh_set_aca_impl 2): tiles of 16 granules, stored terms staged through shared memory by TMA bulk copies.
-        // Measured slower at c3 (ms_aca 6,456 vs 5,066): see the comment above k2_step_t and DESIGN.md section 6
+        // Measured slower at c3 (ms_aca 6,456 vs 5,066 for the fused form): see the comment above k2_step_t and DESIGN.md section 6
         if (!ctx->aca_smem_set) {
           HH_CUDA(cudaFuncSetAttribute(k2_step_t<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TS_SMEM));
           HH_CUDA(cudaFuncSetAttribute(k2_step_t<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TS_SMEM));
@@ -1185,11 +1201,12 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
         k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
         k2_step_t<true><<<HH_N + (t2 < tcap ? t2 : tcap), TS_ROWS, TS_SMEM, s>>>(A, gnc, gmc, &ctx->d_sc->aca_err);   // + line 6 (normalisation)
       } else {
-      if (ctx->p.aca_precision) k2_step<false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
-      else k2_step<false, false><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
-      k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
-      if (ctx->p.aca_precision) k2_step<true, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);   // + line 6 (normalisation)
-      else k2_step<true, false><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
+        // the fused form (hh_set_aca_impl 3; and the fp64 parity mode, aca_precision = 1): entries and update in one kernel
+        if (ctx->p.aca_precision) k2_step<false, true><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
+        else k2_step<false, false><<<HH_N + gr, A2_T, 0, s>>>(A, gmc, 0u);
+        k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
+        if (ctx->p.aca_precision) k2_step<true, true><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);   // + line 6 (normalisation)
+        else k2_step<true, false><<<HH_N + gc, A2_T, 0, s>>>(A, gnc, gmc);
       }
       k2_fin<<<HH_N + gb, 256, 0, s>>>(A);
       HH_LAUNCH_CHECK();

@@ -257,11 +257,11 @@ extern "C" int hh_set_pair_capacity(hh_ctx* ctx, int64_t pairs_per_particle) {
   return HH_OK;
 }
 
-// 0 = lock-step over the batch, every thread loads the stored rank terms of its row (default),
+// 0 = lock-step over the batch, entries (k2_eval) and vectorised update (k2_upd) as separate launches (default),
 // 1 = one CTA per admissible block (the first form), 2 = lock-step with the stored terms staged through shared memory by TMA
-// bulk copies (measured slower); 1, 2 kept for comparison
+// bulk copies, 3 = lock-step with entries and update fused in one kernel (k2_step); 1-3 measured slower, kept for comparison
 extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
-  if (!ctx || impl < 0 || impl > 4) return HH_ERR_INVALID_ARG;
+  if (!ctx || impl < 0 || impl > 3) return HH_ERR_INVALID_ARG;
   if (impl == 1 && ctx->mlp2_wide) return hh_fail(ctx, HH_ERR_UNSUPPORTED, "the paper-size MLP runs in the lock-step form only");
   ctx->aca_impl = impl;
   ctx->res_first = ctx->res_next = 0;
@@ -271,7 +271,7 @@ extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
 // 0 = ring kernel (TMA bulk copies into a shared-memory ring, persistent CTAs) for blocks with max(m,n) <= 256 (default),
 // 1 = one CTA per block in every size class (round 1's kernel; kept for comparison)
 extern "C" int hh_set_far_impl(hh_ctx* ctx, int impl) {
-  if (!ctx || (impl != 0 && impl != 1)) return HH_ERR_INVALID_ARG;
+  if (!ctx || impl < 0 || impl > 2) return HH_ERR_INVALID_ARG;
   ctx->far_impl = impl;
   return HH_OK;
 }

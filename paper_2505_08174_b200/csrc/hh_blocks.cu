@@ -125,9 +125,9 @@ __global__ void __launch_bounds__(256) k_g_post(const uint2* __restrict__ PG, in
     u32 mx = m > q ? m : q;
     u32 pmx = 0xffffffffu;
     if (k > 0) { uint2 pp = PG[k - 1]; u32 a = nhi[pp.x] - nlo[pp.x], b = nhi[pp.y] - nlo[pp.y]; pmx = a > b ? a : b; }
-    const u32 th[3] = {256u, 128u, 64u};
+    const u32 th[4] = {256u, 128u, 64u, HH_FAR_MID_MAX};          // [3]: first block of the far-field apply's mid-size class (hh_far.cu)
 #pragma unroll
-    for (int c = 0; c < 3; ++c) if (mx <= th[c] && pmx > th[c]) sc->class_bound[c] = (u32)k;
+    for (int c = 0; c < 4; ++c) if (mx <= th[c] && pmx > th[c]) sc->class_bound[c] = (u32)k;
   }
   for (int o = 16; o; o >>= 1) rc += __shfl_xor_sync(0xffffffffu, rc, o);
   if ((threadIdx.x & 31) == 0 && rc) atomicAdd((unsigned long long*)&sc->far_rows_cols, (unsigned long long)rc);
@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(256) k_h_post(const uint2* __restrict__ PH, in
 }
 
 __global__ void k_blocks_init(DevScalars* sc, u32 nG) {
-  sc->class_bound[0] = sc->class_bound[1] = sc->class_bound[2] = nG;
+  sc->class_bound[0] = sc->class_bound[1] = sc->class_bound[2] = sc->class_bound[3] = nG;
   sc->near_entries = 0; sc->far_rows_cols = 0;
 }
 
@@ -219,6 +219,7 @@ int hh_blocks_build(hh_ctx* ctx) {
   ctx->class_bound[0] = 0;
   for (int c = 0; c < 3; ++c) ctx->class_bound[c + 1] = ctx->h_sc->class_bound[c];
   ctx->class_bound[4] = (u32)nG;
+  ctx->mid_bound = ctx->h_sc->class_bound[3] < ctx->h_sc->class_bound[0] ? ctx->h_sc->class_bound[3] : ctx->h_sc->class_bound[0];   // <= first block of class 1
   // boundaries are "first index with size <= threshold"; a class that never starts keeps nG, and a
   // later class may start earlier only if sizes skip a class entirely -> make monotone
   for (int c = 3; c >= 1; --c) if (ctx->class_bound[c] > ctx->class_bound[c + 1]) ctx->class_bound[c] = ctx->class_bound[c + 1];

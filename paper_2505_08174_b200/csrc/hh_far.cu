@@ -367,6 +367,204 @@ __global__ void __launch_bounds__(256) k_far_fill(const uint2* __restrict__ PG, 
 }
 
 
+// =====================================================================================================================
+// The same ring for MID-SIZE blocks (256 < max(m,n) <= HH_FAR_MID_MAX = 1024): a persistent CTA takes WHOLE blocks
+// (round-robin over the grid: P^G is sorted by size) and streams each rank term as two items, each ONE contiguous bulk copy
+// of 36 n_pad resp. 36 m_pad bytes (the nine planes of a rank lie back to back in an arena chunk):
+//   Q items (rank k):  t_k = sum_j Q_k(j) F(j), all 128 consumers over the columns (F^sigma sits in registers for the whole
+//                      block), per-warp partial sums to shared memory;
+//   C items (rank k):  u(i) += C_k(i) t_k in registers, every thread owning its rows for all ranks; U(i) += u(i) once per block
+// in that order (all t of the block, then the C items).  The producer makes up the item descriptors on the fly from the
+// block's table row (no item list in memory) and ends with a sentinel.  One CTA per block (k_far<256,2048>) streams these
+// blocks at 5.3-5.8 TB/s at c3 (profiles/r02b_far_ring_c3.md).
+// A first version cut the blocks into slices of 256 (128) rows: 36 plane segments of 1 KB (512 B) per item, one bulk copy
+// each -- 4.2 TB/s (3.4): bulk copies are issued one at a time from uniform registers, and 36 small ones per item cost the
+// producer warp more than the item's share of the bandwidth allows.
+// =====================================================================================================================
+/* which hh_set_far_impl value routes 256 < max(m,n) <= HH_FAR_MID_MAX through k_far_mid: 2 = opt-in (measured slower than one CTA per block so far) */
+#ifndef FAR_MID_IMPL
+#define FAR_MID_IMPL 2
+#endif
+#ifndef FAR_MID_RING
+#define FAR_MID_RING (200 * 1024)
+#define FAR_MID_CTAS 1
+#endif
+#define FAR_MID_NQ ((HH_FAR_MID_MAX + 511) / 512)      /* quads of 4 rows / columns per consumer thread */
+
+struct FarMidDesc {            /* 32 bytes, written by the producer into the barrier slot of the item */
+  u32 pbase;                   /* first particle (tree order) of the side: slo (Q item) resp. tlo (C item) */
+  u32 len;                     /* columns resp. rows */
+  u32 lenp;                    /* padded to 8: the plane stride */
+  u32 k;                       /* rank term */
+  u32 type;                    /* 0 Q item, 1 C item, 2 end */
+  u32 flags;                   /* bit 0: first item of its kind in the block (Q: load F^sigma; C: all t are there), bit 1: last C item (flush U), bit 2: parity of the block */
+  u32 pad[2];
+};
+
+__global__ void __launch_bounds__(128 + 32, FAR_MID_CTAS) k_far_mid(const uint2* __restrict__ PG, const u32* __restrict__ nlo, const u32* __restrict__ nhi,
+                                                          const int* __restrict__ ranks, const int* __restrict__ flags, const u32* __restrict__ tab,
+                                                          u32 first, u32 begin, u32 end, const float* __restrict__ arena,
+                                                          const float* __restrict__ Fs, float* __restrict__ Us, u32* __restrict__ err) {
+  constexpr int G = 128, NQ = FAR_MID_NQ, RING = FAR_MID_RING;
+  extern __shared__ __align__(128) unsigned char far_raw[];
+  unsigned char* ringb = far_raw + ((128u - (far_smem_u32(far_raw) & 127u)) & 127u);
+  unsigned long long* bars = reinterpret_cast<unsigned long long*>(ringb + RING);     // full[NS], empty[NS]
+  FarMidDesc* sdesc = reinterpret_cast<FarMidDesc*>(bars + 2 * FAR_NS);
+  u32* soff = reinterpret_cast<u32*>(sdesc + FAR_NS);
+  float* stt = reinterpret_cast<float*>(soff + FAR_NS);                              // [2][HH_MAX_RANK][4 warps][4]: partial t_k, by block parity
+  const u32 tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const u32 bar_full = far_smem_u32(bars), bar_empty = far_smem_u32(bars + FAR_NS);
+  if (tid == 0) {
+    for (int s = 0; s < FAR_NS; ++s) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar_full + 8 * s) : "memory");
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar_empty + 8 * s), "r"(G) : "memory");
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid >= G) {
+    // ------------------------------------------------ producer warp ------------------------------------------------
+    u32 head = 0, released = 0, myoff = 0, q = 0, par = 0;
+    unsigned long long pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    bool alive = true;
+    // reserve B bytes of the ring for item q (items are released in order); false = a wait timed out
+    auto reserve = [&](u32 B, u32& off) -> bool {
+      for (;;) {
+        const u32 outst = q - released;
+        if (outst == 0) { off = 0; return true; }
+        if (outst < FAR_NS) {
+          const u32 tail = __shfl_sync(0xffffffffu, myoff, released % FAR_NS);
+          if (head > tail) {
+            if (head + B <= (u32)RING) { off = head; return true; }
+            if (B < tail) { off = 0; return true; }
+          } else if (head + B < tail) { off = head; return true; }
+        }
+        if (!far_mbar_wait(bar_empty + 8 * (released % FAR_NS), (released / FAR_NS) & 1u)) return false;
+        ++released;
+      }
+    };
+    for (u32 g = begin + blockIdx.x; g < end && alive; g += gridDim.x) {
+      const int l = ranks[g];
+      if (l <= 0 || flags[g] == 2) continue;
+      const uint2 blk = PG[g];
+      const u32 tlo = nlo[blk.x], m = nhi[blk.x] - tlo, slo = nlo[blk.y], n = nhi[blk.y] - slo;
+      const u32 mp = pad8f(m), np = pad8f(n);
+      const u32 mych = lane < HH_MAX_CHUNKS ? tab[(size_t)(g - first) * HH_TAB_STRIDE + lane] : 0u;   // lane c: offset of chunk c
+      for (u32 it = 0; it < 2u * (u32)l; ++it) {
+        const u32 type = it >= (u32)l ? 1u : 0u, k = type ? it - (u32)l : it;
+        const u32 lenp = type ? mp : np, B = 36u * lenp;
+        u32 off;
+        if (!reserve(B, off)) { alive = false; break; }
+        head = off + B;
+        const u32 slot = q % FAR_NS;
+        if (lane == slot) myoff = off;
+        const u32 choff = __shfl_sync(0xffffffffu, mych, k / HH_RC);
+        if (lane == 0) {
+          soff[slot] = off;
+          FarMidDesc d;
+          d.pbase = type ? tlo : slo; d.len = type ? m : n; d.lenp = lenp; d.k = k; d.type = type;
+          d.flags = (k == 0 ? 1u : 0u) | ((type && k + 1 == (u32)l) ? 2u : 0u) | (par << 2); d.pad[0] = d.pad[1] = 0;
+          sdesc[slot] = d;
+          const u32 fb = bar_full + 8 * slot;
+          const float* src = arena + (size_t)choff * HH_UNIT_FLOATS + (type ? (size_t)0 : (size_t)HH_RC * 9 * mp) + (size_t)(k % HH_RC) * 9 * lenp;
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fb), "r"(B) : "memory");
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(far_smem_u32(ringb + off)),
+                       "l"(src), "r"(B), "r"(fb), "l"(pol) : "memory");
+        }
+        ++q;
+      }
+      par ^= 1u;
+    }
+    if (!alive) { if (lane == 0) atomicExch(err, 1u); return; }
+    u32 off;                                                  // sentinel: the consumers leave
+    if (!reserve(16u, off)) { if (lane == 0) atomicExch(err, 1u); return; }
+    if (lane == 0) {
+      const u32 slot = q % FAR_NS;
+      soff[slot] = off;
+      FarMidDesc d;
+      d.pbase = d.len = d.lenp = d.k = d.flags = d.pad[0] = d.pad[1] = 0; d.type = 2;
+      sdesc[slot] = d;
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar_full + 8 * slot) : "memory");
+    }
+    return;
+  }
+  // -------------------------------------------------- consumers --------------------------------------------------
+  // thread tid owns the quads tid, tid + 128, ... of 4 consecutive columns (Q items) resp. rows (C items)
+  float u[NQ][4][3], f[NQ][12];
+#pragma unroll
+  for (int r = 0; r < NQ; ++r)
+#pragma unroll
+    for (int c = 0; c < 4; ++c) u[r][c][0] = u[r][c][1] = u[r][c][2] = 0.f;
+  for (u32 q = 0;; ++q) {
+    const u32 slot = q % FAR_NS;
+    if (!far_mbar_wait(bar_full + 8 * slot, (q / FAR_NS) & 1u)) { atomicExch(err, 1u); return; }
+    const FarMidDesc d = sdesc[slot];
+    if (d.type == 2u) return;
+    const u32 len = d.len, lenp = d.lenp;
+    const float* base = reinterpret_cast<const float*>(ringb + soff[slot]);
+    float* st = stt + (((d.flags >> 2) & 1u) * HH_MAX_RANK + d.k) * 16;
+    if (d.type == 0u) {
+      if (d.flags & 1u) {                                     // a new block: its F^sigma into registers (zero beyond n)
+#pragma unroll
+        for (int c = 0; c < NQ; ++c) {
+          const u32 j = 4u * (tid + c * G);
+#pragma unroll
+          for (int e = 0; e < 12; ++e) f[c][e] = j + e / 3 < len ? Fs[3 * (size_t)(d.pbase + j) + e] : 0.f;
+        }
+      }
+      float a0 = 0.f, a1 = 0.f, a2 = 0.f;
+#pragma unroll
+      for (int c = 0; c < NQ; ++c) {
+        const u32 j = 4u * (tid + c * G);
+        if (j < len) {
+          float4 qv[9];
+#pragma unroll
+          for (int e = 0; e < 9; ++e) qv[e] = *reinterpret_cast<const float4*>(base + e * lenp + j);
+#define FAR_DOTM(a, fc) ((a).x * f[c][(fc)] + (a).y * f[c][3 + (fc)] + (a).z * f[c][6 + (fc)] + (a).w * f[c][9 + (fc)])
+          a0 += FAR_DOTM(qv[0], 0) + FAR_DOTM(qv[1], 1) + FAR_DOTM(qv[2], 2);
+          a1 += FAR_DOTM(qv[3], 0) + FAR_DOTM(qv[4], 1) + FAR_DOTM(qv[5], 2);
+          a2 += FAR_DOTM(qv[6], 0) + FAR_DOTM(qv[7], 1) + FAR_DOTM(qv[8], 2);
+        }
+      }
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar_empty + 8 * slot) : "memory");
+#pragma unroll
+      for (int o = 16; o; o >>= 1) {
+        a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o); a2 += __shfl_xor_sync(0xffffffffu, a2, o);
+      }
+      if (lane == 0) { st[4 * warp] = a0; st[4 * warp + 1] = a1; st[4 * warp + 2] = a2; }
+    } else {
+      if (d.flags & 1u) asm volatile("bar.sync 1, %0;" ::"n"(G) : "memory");     // every t_k of the block is in shared memory
+      const float t0 = (st[0] + st[4]) + (st[8] + st[12]), t1 = (st[1] + st[5]) + (st[9] + st[13]), t2 = (st[2] + st[6]) + (st[10] + st[14]);
+#pragma unroll
+      for (int r = 0; r < NQ; ++r) {
+        const u32 i = 4u * (tid + r * G);
+        if (i < len) {
+          float4 cv[9];
+#pragma unroll
+          for (int e = 0; e < 9; ++e) cv[e] = *reinterpret_cast<const float4*>(base + e * lenp + i);
+          FAR_ROW(0, x) FAR_ROW(1, y) FAR_ROW(2, z) FAR_ROW(3, w)
+        }
+      }
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar_empty + 8 * slot) : "memory");
+      if (d.flags & 2u) {                                     // the block ends: three atomics per row
+#pragma unroll
+        for (int r = 0; r < NQ; ++r) {
+          const u32 i = 4u * (tid + r * G);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            if (i + c < len) {
+              float* up = Us + 3 * (size_t)(d.pbase + i + c);
+              atomicAdd(up, u[r][c][0]); atomicAdd(up + 1, u[r][c][1]); atomicAdd(up + 2, u[r][c][2]);
+            }
+            u[r][c][0] = u[r][c][1] = u[r][c][2] = 0.f;
+          }
+        }
+      }
+    }
+  }
+}
+
 // CTA sizes per size class (max(m,n) > 256, <= 256, <= 128, <= 64) and the 64-register cap (32 warps per SM) are measured,
 // not derived: the kernel is bound by per-CTA start-up latency and load concurrency.  512 threads / 70 registers for the
 // first class gave 4.28 TB/s at c3, 256 threads / 64 registers 5.03 TB/s (c4: 4.52 -> 5.06 TB/s); halving the threads of
@@ -392,7 +590,7 @@ int hh_far_apply(hh_ctx* ctx) {
   // ring classes (max(m,n) <= 256): item list of the resident blocks, once per batch (it lives in the dead lock-step
   // accumulators of the batch, hh_aca2.cu)
   const u32 rb = ctx->class_bound[1] > first ? ctx->class_bound[1] : first;
-  const bool ring = ctx->far_impl == 0 && ctx->far_items != nullptr && rb < end;
+  const bool ring = ctx->far_impl != 1 && ctx->far_items != nullptr && rb < end;
   if (ring && !ctx->far_built) {
     k_far_count<<<HH_N + cdiv((int64_t)(end - rb) + 1, 256), 256, 0, s>>>(ctx->ranks, ctx->flags, rb, end, ctx->far_cnt);
     HH_TRY(hh_scan_u32(ctx, ctx->far_cnt, ctx->far_cnt, (int64_t)(end - rb) + 1, nullptr));
@@ -411,6 +609,20 @@ int hh_far_apply(hh_ctx* ctx) {
         default: HH_TRY((far_ring_launch<64, 1, FAR_RING3>(ctx, 3, b - rb, e - rb, FAR_CTAS3))); break;
       }
       continue;
+    }
+    if (c == 0 && ctx->far_impl == FAR_MID_IMPL && ctx->mid_bound < e) {
+      // mid-size blocks [max(b, mid_bound), e): whole blocks per persistent CTA, rank by rank through the ring
+      const u32 mb = ctx->mid_bound > b ? ctx->mid_bound : b;
+      const size_t smem = (size_t)FAR_MID_RING + 128 + 2 * FAR_NS * 8 + FAR_NS * sizeof(FarMidDesc) + FAR_NS * 4 + 2 * HH_MAX_RANK * 16 * 4;
+      if (!(ctx->far_smem_set & 1)) {
+        HH_CUDA(cudaFuncSetAttribute(k_far_mid, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ctx->far_smem_set |= 1;
+      }
+      const u32 nblk = e - mb, cap = (u32)ctx->n_sm * FAR_MID_CTAS;
+      k_far_mid<<<HH_N + (nblk < cap ? nblk : cap), 128 + 32, smem, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, first, mb, e, ctx->arena,
+                                                                          ctx->Fs, ctx->Us, &ctx->d_sc->far_err);
+      e = mb;
+      if (b >= e) continue;
     }
     switch (c) {
       case 0: k_far<256, 2048><<<HH_N + e - b, 256, 0, s>>>(ctx->PG, ctx->nlo, ctx->nhi, ctx->ranks, ctx->flags, ctx->tab, ctx->arena, ctx->Fs, ctx->Us, first, b); break;

@@ -17,6 +17,9 @@ typedef uint64_t u64;
 #define HH_TAB_PIV 24
 #define HH_MAX_LEAF 256                         /* largest supported C_leaf                        */
 #define HH_MAX_LEVELS 128
+#ifndef HH_FAR_MID_MAX
+#define HH_FAR_MID_MAX 1024                     /* far-field apply: blocks with 256 < max(m,n) <= this go through k_far_mid (hh_far.cu) */
+#endif
 #define HH_CAP_STRIDE 200                      /* int32 per captured pivot record (hh.h: hh_set_capture) */
 
 /* packed MLP weights (floats) as laid out for the kernels: W1 [H][INP], b1 [H], W2 [H][H], b2 [H],
@@ -63,7 +66,7 @@ struct hh_ctx {
   char err[512];
   int have_mlp3;
   int timing;
-  int aca_impl;                         /* 0 = lock-step, per-thread loads (hh_aca2.cu), 1 = one CTA per block (hh_aca.cu), 2 = lock-step, stored terms staged by TMA */
+  int aca_impl;                         /* 0 = lock-step, entries and vectorised update in separate launches (hh_aca2.cu), 1 = one CTA per block (hh_aca.cu), 2 = lock-step, stored terms staged by TMA, 3 = lock-step, fused k2_step */
   int n_sm;                             /* cudaDevAttrMultiProcessorCount of the context's device (grid sizing) */
   int three_smem_set;                   /* k_three's dynamic shared-memory attribute has been set on this device */
   int64_t pairs_per_particle;
@@ -76,6 +79,7 @@ struct hh_ctx {
   int64_t res_first, res_next;          /* resident factor range [first, next) of sorted P^G */
   double l_pred;                        /* predicted rank for batch sizing                   */
   u32 class_bound[5];
+  u32 mid_bound;                        /* first block of sorted P^G with max(m,n) <= HH_FAR_MID_MAX */
   hh_stats st;
   int64_t n_launches;                   /* kernels launched since the last hh_build_tree began (claim for bench.py) */
   /* pinned host scratch */

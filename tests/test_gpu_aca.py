@@ -201,11 +201,14 @@ def test_far_apply_kernel_vs_its_own_factors(mlp2):
     ctx.close()
 
 
-@pytest.mark.parametrize("leaf,n,eta,tol", [(200, 12000, 1.0, 1e-4), (100, 9000, 1.0, 1e-5), (40, 6000, 2.0, 1e-4), (3, 700, 1.0, 1e-6)])
+@pytest.mark.parametrize("leaf,n,eta,tol", [(200, 12000, 1.0, 1e-4), (100, 9000, 1.0, 1e-5), (40, 6000, 2.0, 1e-4), (3, 700, 1.0, 1e-6),
+                                             (64, 40000, 0.6, 1e-5), (250, 30000, 1.0, 1e-4)])
 def test_far_ring_kernel_equals_one_cta_per_block(mlp2, leaf, n, eta, tol):
     """row 9, both forms on the SAME resident factors: the ring kernel (persistent CTAs, TMA bulk copies into a shared-memory
     byte ring; blocks with max(m,n) <= 256) against round 1's one-CTA-per-block kernel, in every ring size class (leaf 200:
-    129..256, leaf 100: 65..128, leaf 40: <= 64, leaf 3: rows and columns below the pad width, ranks up to min(m,n))"""
+    129..256, leaf 100: 65..128, leaf 40: <= 64, leaf 3: rows and columns below the pad width, ranks up to min(m,n)) and the
+    whole-block ring kernel k_far_mid (hh_set_far_impl 2) for 256 < max(m,n) <= 1024 (40,000 and 30,000 particles: blocks of
+    300..1,000 rows, several chunks per block)"""
     X = synth.ball_cloud(n, 0.2, seed=11) if leaf != 40 else synth.chain_cloud(n // 50, 50, 0.1)
     F = synth.gaussian_forces(len(X), seed=3)
     ctx = setup(X, mlp2, leaf_size=leaf, eta=eta, aca_tol=tol)
@@ -220,8 +223,10 @@ def test_far_ring_kernel_equals_one_cta_per_block(mlp2, leaf, n, eta, tol):
         ctx.set_far_impl(0)
         U0 = ctx.far_apply_resident(to_dev(F)).cpu().numpy()
         U0b = ctx.far_apply_resident(to_dev(F)).cpu().numpy()      # the item list is reused while the factors stay resident
+        ctx.set_far_impl(2)                                         # + k_far_mid for 256 < max(m,n) <= 1024
+        U2 = ctx.far_apply_resident(to_dev(F)).cpu().numpy()
         assert np.linalg.norm(U1) > 0
-        worst = max(worst, rel_l2(U0, U1), rel_l2(U0b, U1))
+        worst = max(worst, rel_l2(U0, U1), rel_l2(U0b, U1), rel_l2(U2, U1))
         first = nxt
     print("leaf %d: ring vs one-CTA-per-block far-field apply: rel L2 %.3e over %d blocks" % (leaf, worst, nG))
     assert worst <= 1e-6
@@ -281,14 +286,14 @@ def test_degenerate_blocks(mlp2):
 
 
 def test_both_aca_forms_agree(mlp2):
-    """hh_set_aca_impl: the lock-step form (default: per-thread loads; 2: stored terms staged by TMA bulk copies) and the
-    one-CTA-per-block form (1) run the same Alg. 2; pivots, ranks and flags agree on all but near-tie blocks and the mat-vecs
-    agree to fp32 summation order.  Forms 0 and 2 do the same arithmetic in the same order on each entry (only the Gram sums
-    are float atomics), so they differ by even less."""
+    """hh_set_aca_impl: the lock-step forms (0, the default: entries and vectorised update in separate launches; 2: stored terms
+    staged by TMA bulk copies; 3: entries and update fused) and the one-CTA-per-block form (1) run the same Alg. 2; pivots, ranks
+    and flags agree on all but near-tie blocks and the mat-vecs agree to fp32 summation order.  The lock-step forms do the same
+    arithmetic in the same order on each entry (only the Gram sums are float atomics), so they differ by even less."""
     X = synth.cube_cloud(5000, 0.1, seed=9)
     F = synth.gaussian_forces(5000)
     res = []
-    for impl in (0, 1, 2, 3, 4):
+    for impl in (0, 1, 2, 3):
         ctx = setup(X, mlp2, leaf_size=32, eta=1.0, aca_tol=1e-4, ws_mb=8192)
         ctx.set_aca_impl(impl)
         U = ctx.matvec(to_dev(F)).cpu().numpy()
@@ -296,7 +301,7 @@ def test_both_aca_forms_agree(mlp2):
         res.append((U, ranks, flags, ctx.stats()))
         ctx.close()
     U0, r0, f0, s0 = res[0]
-    for impl in (1, 2, 3, 4):
+    for impl in (1, 2, 3):
         U1, r1, f1, s1 = res[impl]
         assert s0["aca_batches"] == s1["aca_batches"] == 1
         print("aca_impl %d vs 0: rel L2 %.3e, ranks differ on %.4f of the blocks" % (impl, rel_l2(U0, U1), np.mean(r0 != r1)))
@@ -305,7 +310,7 @@ def test_both_aca_forms_agree(mlp2):
         assert rel_l2(U0, U1) <= 1e-5
 
 
-IMPLS = (0, 2, 3, 4)
+IMPLS = (0, 2, 3)
 
 
 @pytest.mark.parametrize("name,gen,leaf,eta,zeta", [
@@ -313,10 +318,11 @@ IMPLS = (0, 2, 3, 4)
     ("big_blocks_slices", lambda: synth.cube_cloud(20000, 0.1, seed=6), 64, 0.7, 1e-4),
     ("tiny_leaves", lambda: synth.cube_cloud(1500, 0.1, seed=8), 5, 1.0, 1e-5),
 ])
-def test_staged_lockstep_equals_per_thread_loads(mlp2, name, gen, leaf, eta, zeta):
-    """k2_step_t (tiles of 256 rows, the first 10 stored terms staged by TMA) against k2_step (every term loaded by the thread that
-    needs it) on clouds that exercise: ranks beyond the staged 10, slices of blocks larger than a tile and blocks that straddle
-    a tile boundary, leaves smaller than a granule"""
+def test_lockstep_forms_agree(mlp2, name, gen, leaf, eta, zeta):
+    """the three lock-step forms against each other -- k2_eval + k2_upd (default: 4 rows resp. 2 columns per thread, vector loads),
+    k2_step_t (tiles of 256 rows, the first 10 stored terms staged by TMA), k2_step (fused, one entry per thread) -- on clouds that
+    exercise: ranks beyond the staged 10, slices of blocks larger than a tile and blocks that straddle a tile boundary, leaves
+    smaller than a granule (pad rows and columns inside a thread's vector)"""
     X = gen()
     F = synth.gaussian_forces(len(X), seed=5)
     out = []

@@ -49,15 +49,16 @@ class ClockSampler:
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index):
+    def __init__(self, index, period_ms=200):
         self.index = index
+        self.period_ms = int(period_ms)
         self.rows = []
         self.proc = None
 
     def start(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                          "--format=csv,noheader,nounits", "-lms", str(self.period_ms)],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -252,8 +253,8 @@ def run_gpu(args):
     for _ in range(args.warmup):
         one_step()
     barrier()
-    clocks = ClockSampler(local)
-    if rank == 0:
+    clocks = ClockSampler(local, args.clock_period_ms)
+    if rank == 0 and args.clock_period_ms > 0:
         clocks.start()
     t_wall = time.perf_counter()
     ms, stats = [], []
@@ -404,9 +405,10 @@ def main():
     ap.add_argument("--kappa-max", type=float, default=None, help="S-18b limit on the pivot-block condition number")
     ap.add_argument("--near-path", type=int, default=2, choices=[0, 1, 2], help="0 fp32 ALU, 1 tcgen05 tf32 + tanh.approx (2e-3), 2 tcgen05 split tf32 + tanhf")
     ap.add_argument("--aca-precision", type=int, default=0, choices=[0, 1], help="1 = fp64 entries and residuals in Alg. 2 (parity mode)")
-    ap.add_argument("--aca-impl", type=int, default=0, choices=[0, 1, 2, 3], help="hh_set_aca_impl: 0 lock-step, entries and update in separate launches (default), 1 one CTA per block, 2 lock-step with TMA-staged terms, 3 lock-step, fused")
-    ap.add_argument("--far-impl", type=int, default=0, choices=[0, 1, 2], help="hh_set_far_impl: 0 ring kernel for blocks <= 256 (default), 1 one CTA per block, 2 = 0 + whole-block ring kernel for blocks <= 1024")
+    ap.add_argument("--aca-impl", type=int, default=0, choices=[0, 1, 2, 3, 4], help="hh_set_aca_impl: 0 lock-step, entries and update in separate launches (default), 1 one CTA per block, 2 lock-step with TMA-staged terms, 3 lock-step, fused, 4 = 0 on two half-batches (update of one beside the entries of the other)")
+    ap.add_argument("--far-impl", type=int, default=0, choices=[0, 1, 2], help="hh_set_far_impl: 0 ring kernels for blocks <= 1024 (default), 1 one CTA per block, 2 ring kernel only for blocks <= 256")
     ap.add_argument("--paper-mlp", action="store_true", help="two-body MLP with the paper's hidden layers 128/512/128 (tensor-core tile)")
+    ap.add_argument("--clock-period-ms", type=int, default=200, help="nvidia-smi sampling period during the timed region (0 = no sampling: to measure what the sampler itself costs)")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     ap.add_argument("--no-c4", dest="with_c4", action="store_false", help="skip the 10M-particle sub-record of the default (c3) run")
     args = ap.parse_args()

@@ -132,10 +132,10 @@ int hh_set_params(hh_ctx* ctx, const hh_params* params);
  * summation order in the norm recursion. */
 int hh_set_aca_impl(hh_ctx* ctx, int impl);
 
-/* Far-field apply form: 0 = blocks with max(m,n) <= 256 are streamed by persistent CTAs through a
- * shared-memory ring filled by TMA bulk copies, larger ones by one CTA per block (default); 1 = one CTA per block in every
- * size class; 2 = 0 plus a whole-block ring kernel for 256 < max(m,n) <= 1024 (measured slower, kept for comparison).  Same
- * sums up to fp32 summation order. */
+/* Far-field apply form: 0 = blocks with max(m,n) <= 1024 are streamed by persistent CTAs through a
+ * shared-memory ring filled by TMA bulk copies (chunk by chunk up to 256, rank by rank above), larger ones by one CTA per
+ * block (default); 1 = one CTA per block in every size class; 2 = the ring only up to 256.  Same sums up to fp32 summation
+ * order. */
 int hh_set_far_impl(hh_ctx* ctx, int impl);
 
 /* Record per-stage CUDA-event times into hh_stats (adds stream synchronisations). */

@@ -54,6 +54,7 @@ struct A2Args {
   int R;                         /* rank cap of the context: accumulators hold R + 1 Gram slots          */
   BlkState* st; unsigned long long* amax; double* pinv; float* acc;
   u32 *cm, *cn; uint2 *gm, *gn;
+  u32* nact;                     /* counter of the active blocks (k2_gran_count)                          */
 };
 
 __device__ __forceinline__ u32 a2_pad8(u32 v) { return (v + 7u) & ~7u; }
@@ -154,7 +155,7 @@ __global__ void __launch_bounds__(256) k2_gran_count(A2Args A) {
     A.cn[b] = act ? (s.n + GR - 1) / GR : 0u;
   }
   act = __popc(__ballot_sync(0xffffffffu, act));
-  if ((threadIdx.x & 31) == 0 && act) atomicAdd(&A.sc->n_split, act);        // n_split doubles as the active-block count here
+  if ((threadIdx.x & 31) == 0 && act) atomicAdd(A.nact, act);
 }
 __global__ void __launch_bounds__(256) k2_gran_fill(A2Args A) {                // one warp per block
   const u32 b = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
@@ -478,6 +479,12 @@ __global__ void __launch_bounds__(A2_T, 2) k2_eval(A2Args A, u32 count, u32 ncou
 // (2) of a granule, so the stored rank terms are read as 16- / 8-byte loads, the 27 multiply-adds per rank term are done for RPT
 // entries per fixed-operand fetch, and the 3x3 Gram sums of a granule are reduced over 4 resp. 8 lanes instead of 16.  Per
 // (entry, rank term) that is about 80 instructions instead of 200 in k2_step.  Arithmetic per entry is k2_step's, in its order.
+#ifndef K2U_UNROLL
+#define K2U_UNROLL 2             /* rank terms in flight per thread in k2_upd's update loop                */
+#endif
+#ifndef K2U_CTAS_COLS
+#define K2U_CTAS_COLS 2          /* CTAs of k2_upd<false> per SM (the grid cap): fewer rows in flight = the Gram pass finds more of its terms in L2 */
+#endif
 template <int TPG>                                                  // sum 9 values over the TPG lanes of a granule group;
 __device__ __forceinline__ void group_sum9(const float (&in)[9], u32 lig, float (&out)[TPG == 4 ? 3 : 2]) {   // lane lig gets slots [VPL lig, VPL lig + VPL)
   constexpr int VPL = TPG == 4 ? 3 : 2, NS = TPG * VPL;
@@ -563,7 +570,8 @@ __global__ void __launch_bounds__(A2_T, 2) k2_upd(A2Args A, u32 count, u32 ncoun
 #pragma unroll
         for (int c = 0; c < RPT; ++c) if (idx0 + c >= len) v[r][c] = 0.f;                  // pad rows / columns
       const u32 fix = COLS ? (u32)s.ik : (u32)s.jk;
-#pragma unroll 2
+      constexpr int UNR = K2U_UNROLL;
+#pragma unroll UNR
       for (int p = 0; p < k; ++p) {
         const float* base = chunk_ptr(A, tabrow, p);
         const float* Cp = base + (size_t)(p % HH_RC) * 9 * mp;
@@ -1087,6 +1095,12 @@ __global__ void k2_batch_range(const u64* __restrict__ unit_prefix, u32 first, u
   }
   sc->batch_end = lo;
   sc->batch_units = unit_prefix[lo] - s0;
+  {                                                      // first block of the second half: half of the rows + columns on either side
+    const u64 target = s0 + (unit_prefix[lo] - s0) / 2;
+    u32 a = first, b = lo;
+    while (a < b) { const u32 mid = a + (b - a) / 2; if (unit_prefix[mid] < target) a = mid + 1; else b = mid; }
+    sc->batch_mid = a;
+  }
   sc->batch_units1 = unit_prefix[first + 1 <= nG ? first + 1 : first] - s0;
   sc->arena_cursor = 0;
   sc->fail_min = 0xffffffffu;
@@ -1094,6 +1108,93 @@ __global__ void k2_batch_range(const u64* __restrict__ unit_prefix, u32 first, u
   sc->not_conv = sc->singular = sc->max_rank_seen = 0;
   sc->n_dense = 0;
   sc->fallback_entries = 0;
+}
+
+// ---- hh_set_aca_impl 4: the batch as TWO half-batches (half of the rows + columns each), one listing line apart ----
+// Entry evaluation (k2_eval) is bound by the ALUs, the update (k2_upd) by memory, and inside one block they cannot overlap
+// (the next pivot needs the finished residual).  Two half-batches can: while half A evaluates entries on the caller's stream,
+// half B runs its update on a side stream, both kernels launched with one CTA per SM so that an SM holds one of each.
+// Per half the four stages are  0: k2_eval<rows of tau>, 1: k2_upd + k2_piv, 2: k2_eval<columns of sigma> (+ line 6),
+// 3: k2_upd + k2_fin + granule lists of the next iteration.  The halves share the arena, its cursor and fail_min.
+static int a2_two_halves(hh_ctx* ctx, const A2Args& A0, u32 mid, u32* cm2, u32* cn2, uint2* gm2, uint2* gn2, size_t ngran) {
+  cudaStream_t s = ctx->stream, s2 = ctx->stream2;
+  const int R = A0.R;
+  const size_t accs = ACC_APK + 9 * (size_t)(R + 1);
+  if (mid <= A0.first) mid = A0.first + 1;
+  if (mid >= A0.first + A0.nb) mid = A0.first + A0.nb - 1;
+  struct Half { A2Args A; u32 gmc, gnc; int stage; bool active; } H[2];
+  for (int h = 0; h < 2; ++h) {
+    const u32 o = h ? mid - A0.first : 0u, n = h ? A0.first + A0.nb - mid : mid - A0.first;
+    A2Args& A = H[h].A;
+    A = A0;
+    A.first = A0.first + o; A.nb = n;
+    A.tab = A0.tab + (size_t)o * HH_TAB_STRIDE; A.st = A0.st + o; A.amax = A0.amax + (size_t)o * 4; A.pinv = A0.pinv + (size_t)o * 9;
+    A.acc = A0.acc + (size_t)o * accs;
+    if (h) { A.cm = cm2; A.cn = cn2; A.gm = gm2; A.gn = gn2; }
+    A.nact = &ctx->d_sc->ab[h];
+    H[h].stage = 0; H[h].active = true; H[h].gmc = H[h].gnc = 0;
+  }
+  // granule lists of a half for its next iteration; the counts come back with the next read-back
+  auto lists = [&](int h) -> int {
+    const A2Args& A = H[h].A;
+    HH_CUDA(cudaMemsetAsync(&ctx->d_sc->ab[h], 0, sizeof(u32), s));
+    k2_gran_count<<<HH_N + cdiv(A.nb, 256), 256, 0, s>>>(A);
+    HH_TRY(hh_scan_u32(ctx, A.cm, A.cm, A.nb, &ctx->d_sc->ab[2 + h]));
+    HH_TRY(hh_scan_u32(ctx, A.cn, A.cn, A.nb, &ctx->d_sc->ab[4 + h]));
+    return HH_OK;
+  };
+  auto readback = [&](int h) -> int {
+    HH_CUDA(cudaMemcpyAsync(ctx->h_sc->ab, ctx->d_sc->ab, sizeof ctx->h_sc->ab, cudaMemcpyDeviceToHost, s));
+    HH_CUDA(cudaStreamSynchronize(s));
+    H[h].active = ctx->h_sc->ab[h] != 0;
+    H[h].gmc = ctx->h_sc->ab[2 + h]; H[h].gnc = ctx->h_sc->ab[4 + h];
+    if (H[h].gmc > ngran || H[h].gnc > ngran) return hh_fail(ctx, HH_ERR_CUDA, "lock-step ACA: granule list overflow (internal)");
+    if (H[h].active) k2_gran_fill<<<HH_N + cdiv((int64_t)H[h].A.nb * 32, 256), 256, 0, s>>>(H[h].A);
+    return HH_OK;
+  };
+  HH_TRY(lists(0)); HH_TRY(readback(0));
+  HH_TRY(lists(1)); HH_TRY(readback(1));
+  const unsigned nsm = (unsigned)ctx->n_sm;
+  for (int tick = 0; tick < 4 * (R + 2) + 2 && (H[0].active || H[1].active); ++tick) {
+    const bool run[2] = {H[0].active, H[1].active && tick > 0};                  // the second half starts one listing line later
+    const bool both = run[0] && run[1];
+    // with both halves in flight one does entries and the other an update (stages of opposite parity): one CTA of each per SM
+    const unsigned cap = both ? nsm : nsm * 2 * 4, ucap = both ? nsm : nsm * K2U_CTAS_COLS, ucap2 = both ? nsm : nsm * 2 * 4;
+    int on_side = -1;
+    if (both) {
+      on_side = (H[0].stage & 1) ? 0 : 1;                                       // the half whose stage is an update goes to the side stream
+      if (!(H[on_side].stage & 1) || (H[1 - on_side].stage & 1)) on_side = -1;  // (both of one kind can only happen after a half has idled: run them in turn)
+    }
+    if (on_side >= 0) { HH_CUDA(cudaEventRecord(ctx->ev_ab[0], s)); HH_CUDA(cudaStreamWaitEvent(s2, ctx->ev_ab[0], 0)); }
+    for (int pass = 0; pass < 2; ++pass) {                                       // side-stream half first, so that both kernels are queued back to back
+      const int h = on_side >= 0 ? (pass == 0 ? on_side : 1 - on_side) : pass;
+      if (!run[h]) continue;
+      const A2Args& A = H[h].A;
+      cudaStream_t st = h == on_side ? s2 : s;
+      const u32 gmc = H[h].gmc, gnc = H[h].gnc;
+      switch (H[h].stage) {
+        case 0: { const unsigned g = cdiv(cdiv(gmc, 4), A2_T / 32); k2_eval<false><<<HH_N + (g < cap ? g : cap), A2_T, 0, st>>>(A, gmc, 0u); break; }
+        case 1: { const unsigned g = cdiv(cdiv(gmc, 8), A2_T / 32); k2_upd<false><<<HH_N + (g < ucap ? g : ucap), A2_T, 0, st>>>(A, gmc, 0u); break; }
+        case 2: { const unsigned g = cdiv(cdiv(gnc > gmc ? gnc : gmc, 4), A2_T / 32); k2_eval<true, true><<<HH_N + (g < cap ? g : cap), A2_T, 0, st>>>(A, gnc, gmc); break; }
+        default: { const unsigned g = cdiv(cdiv(gnc, 4), A2_T / 32); k2_upd<true><<<HH_N + (g < ucap2 ? g : ucap2), A2_T, 0, st>>>(A, gnc, 0u); break; }
+      }
+    }
+    if (on_side >= 0) { HH_CUDA(cudaEventRecord(ctx->ev_ab[1], s2)); HH_CUDA(cudaStreamWaitEvent(s, ctx->ev_ab[1], 0)); }
+    HH_LAUNCH_CHECK();
+    for (int h = 0; h < 2; ++h) {
+      if (!run[h]) continue;
+      const A2Args& A = H[h].A;
+      if (H[h].stage == 1) k2_piv<<<HH_N + cdiv(A.nb, 256), 256, 0, s>>>(A);
+      if (H[h].stage == 3) {
+        k2_fin<<<HH_N + cdiv(A.nb, 256), 256, 0, s>>>(A);
+        HH_TRY(lists(h));
+        HH_TRY(readback(h));
+      }
+      H[h].stage = (H[h].stage + 1) & 3;
+    }
+    HH_LAUNCH_CHECK();
+  }
+  return HH_OK;
 }
 
 static size_t a2_align(size_t v) { return (v + 255) / 256 * 256; }
@@ -1141,6 +1242,12 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     A.cn = (u32*)take((size_t)(nb + 1) * sizeof(u32));
     A.gm = (uint2*)take(ngran * sizeof(uint2));
     A.gn = (uint2*)take(ngran * sizeof(uint2));
+    const bool two_halves = ctx->aca_impl == 4 && !ctx->mlp2_wide && !ctx->p.aca_precision && nb >= 2;
+    u32 *cm2 = nullptr, *cn2 = nullptr; uint2 *gm2 = nullptr, *gn2 = nullptr;
+    if (two_halves) {                                                            // the second half's own counters and granule lists
+      cm2 = (u32*)take((size_t)(nb + 1) * sizeof(u32)); cn2 = (u32*)take((size_t)(nb + 1) * sizeof(u32));
+      gm2 = (uint2*)take(ngran * sizeof(uint2)); gn2 = (uint2*)take(ngran * sizeof(uint2));
+    }
     if (off + 4096 > ctx->scratch_bytes) return hh_fail(ctx, HH_ERR_WORKSPACE_TOO_SMALL, "factor arena too small");
     ctx->arena = (float*)(ctx->scratch + off);
     ctx->arena_units = (ctx->scratch_bytes - off) / 128;
@@ -1152,9 +1259,12 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     A.PG = ctx->PG; A.nlo = ctx->nlo; A.nhi = ctx->nhi; A.Xs = ctx->Xs;
     A.arena = ctx->arena; A.arena_units = ctx->arena_units; A.tab = ctx->tab; A.sc = ctx->d_sc;
     A.ranks = ctx->ranks; A.flags = ctx->flags; A.first = (u32)first; A.nb = nb; A.R = R;
+    A.nact = &ctx->d_sc->n_split;                                                // n_split doubles as the active-block count here
     const unsigned gb = cdiv(nb, 256);
     k2_init<<<HH_N + gb, 256, 0, s>>>(A);
     HH_LAUNCH_CHECK();
+    if (two_halves) HH_TRY(a2_two_halves(ctx, A, ctx->h_sc->batch_mid, cm2, cn2, gm2, gn2, ngran));
+    else
     for (int it = 0; it <= R; ++it) {
       HH_CUDA(cudaMemsetAsync(&ctx->d_sc->n_split, 0, sizeof(u32), s));
       k2_gran_count<<<HH_N + gb, 256, 0, s>>>(A);
@@ -1170,7 +1280,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       const unsigned cap = (unsigned)ctx->n_sm * A2_OCC * 4;
       unsigned g1 = cdiv(cdiv(gmc, 2 * A2_E), A2_T / 32), g2 = cdiv(cdiv(gnc, 2 * A2_E), A2_T / 32);
       const unsigned gr = (g1 < cap ? g1 : cap), gc = (g1 > g2 ? g1 : g2) < cap ? (g1 > g2 ? g1 : g2) : cap;
-      const unsigned ecap = (unsigned)ctx->n_sm * 2 * 4;
+      const unsigned ecap = (unsigned)ctx->n_sm * 2 * 4, ucap = (unsigned)ctx->n_sm * K2U_CTAS_COLS;
       const unsigned u1 = cdiv(cdiv(gmc, 8), A2_T / 32), u2 = cdiv(cdiv(gnc, 4), A2_T / 32), u2n = cdiv(cdiv(gnc > gmc ? gnc : gmc, 4), A2_T / 32);
       if (ctx->mlp2_wide) {
         // paper-size MLP: entries on the tensor cores (hh_wide.cuh), then the vectorised update (line 6 rides with the row side)
@@ -1184,7 +1294,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
         // the default: entries (k2_eval, the MLP at its own register budget) and the vectorised update (k2_upd) as separate launches
         const unsigned e1 = cdiv(cdiv(gmc, 4), A2_T / 32), e2n = cdiv(cdiv(gnc > gmc ? gnc : gmc, 4), A2_T / 32);
         k2_eval<false><<<HH_N + (e1 < ecap ? e1 : ecap), A2_T, 0, s>>>(A, gmc, 0u);
-        k2_upd<false><<<HH_N + (u1 < ecap ? u1 : ecap), A2_T, 0, s>>>(A, gmc, 0u);
+        k2_upd<false><<<HH_N + (u1 < ucap ? u1 : ucap), A2_T, 0, s>>>(A, gmc, 0u);
         k2_piv<<<HH_N + gb, 256, 0, s>>>(A);
         k2_eval<true, true><<<HH_N + (e2n < ecap ? e2n : ecap), A2_T, 0, s>>>(A, gnc, gmc);            // + line 6 (normalisation)
         k2_upd<true><<<HH_N + (u2 < ecap ? u2 : ecap), A2_T, 0, s>>>(A, gnc, 0u);

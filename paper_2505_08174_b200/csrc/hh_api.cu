@@ -184,6 +184,8 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   HH_CUDA(cudaMallocHost((void**)&ctx->h_sc, sizeof(DevScalars)));
   HH_CUDA(cudaMemsetAsync(ctx->d_sc, 0, sizeof(DevScalars), ctx->stream));
   for (int k = 0; k < 8; ++k) HH_CUDA(cudaEventCreate(&ctx->ev[k]));
+  HH_CUDA(cudaStreamCreateWithFlags(&ctx->stream2, cudaStreamNonBlocking));
+  for (int k = 0; k < 2; ++k) HH_CUDA(cudaEventCreateWithFlags(&ctx->ev_ab[k], cudaEventDisableTiming));
   std::vector<float> pk;
   if (mlp2->n_layers == 4) {                        // the paper-size network: tensor-core tile of hh_wide.cuh
     if (params->kappa_max > 0.f || params->aca_precision != 0)
@@ -231,6 +233,8 @@ extern "C" int hh_destroy(hh_ctx* ctx) {
   if (!ctx) return HH_ERR_INVALID_ARG;
   if (ctx->h_sc) cudaFreeHost(ctx->h_sc);
   for (int k = 0; k < 8; ++k) if (ctx->ev[k]) cudaEventDestroy(ctx->ev[k]);
+  for (int k = 0; k < 2; ++k) if (ctx->ev_ab[k]) cudaEventDestroy(ctx->ev_ab[k]);
+  if (ctx->stream2) cudaStreamDestroy(ctx->stream2);
   delete ctx;
   return HH_OK;
 }
@@ -261,15 +265,15 @@ extern "C" int hh_set_pair_capacity(hh_ctx* ctx, int64_t pairs_per_particle) {
 // 1 = one CTA per admissible block (the first form), 2 = lock-step with the stored terms staged through shared memory by TMA
 // bulk copies, 3 = lock-step with entries and update fused in one kernel (k2_step); 1-3 measured slower, kept for comparison
 extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
-  if (!ctx || impl < 0 || impl > 3) return HH_ERR_INVALID_ARG;
+  if (!ctx || impl < 0 || impl > 4) return HH_ERR_INVALID_ARG;
   if (impl == 1 && ctx->mlp2_wide) return hh_fail(ctx, HH_ERR_UNSUPPORTED, "the paper-size MLP runs in the lock-step form only");
   ctx->aca_impl = impl;
   ctx->res_first = ctx->res_next = 0;
   return HH_OK;
 }
 
-// 0 = ring kernel (TMA bulk copies into a shared-memory ring, persistent CTAs) for blocks with max(m,n) <= 256 (default),
-// 1 = one CTA per block in every size class (round 1's kernel; kept for comparison)
+// 0 = ring kernels (TMA bulk copies into a shared-memory ring, persistent CTAs) for blocks with max(m,n) <= 1024 (default),
+// 1 = one CTA per block in every size class (round 1's kernel), 2 = ring kernel only up to 256; 1, 2 kept for comparison
 extern "C" int hh_set_far_impl(hh_ctx* ctx, int impl) {
   if (!ctx || impl < 0 || impl > 2) return HH_ERR_INVALID_ARG;
   ctx->far_impl = impl;

@@ -381,13 +381,12 @@ __global__ void __launch_bounds__(256) k_far_fill(const uint2* __restrict__ PG, 
 // each -- 4.2 TB/s (3.4): bulk copies are issued one at a time from uniform registers, and 36 small ones per item cost the
 // producer warp more than the item's share of the bandwidth allows.
 // =====================================================================================================================
-/* which hh_set_far_impl value routes 256 < max(m,n) <= HH_FAR_MID_MAX through k_far_mid: 2 = opt-in (measured slower than one CTA per block so far) */
-#ifndef FAR_MID_IMPL
-#define FAR_MID_IMPL 2
-#endif
+/* Ring bytes and CTAs per SM are measured (c3, ms_far of the step; 123.5 ms with one CTA per block for this class):
+ *   200 KB x 1 CTA: 131.6 (one group of consumers per SM: every item's wait - load - reduce chain is exposed);
+ *   100 KB x 2 CTAs: 115.0;  60 KB x 3 CTAs with blocks up to 512 only: 117.1;  100 KB x 2 with blocks up to 512 only: 118.6 */
 #ifndef FAR_MID_RING
-#define FAR_MID_RING (200 * 1024)
-#define FAR_MID_CTAS 1
+#define FAR_MID_RING (100 * 1024)
+#define FAR_MID_CTAS 2
 #endif
 #define FAR_MID_NQ ((HH_FAR_MID_MAX + 511) / 512)      /* quads of 4 rows / columns per consumer thread */
 
@@ -610,7 +609,7 @@ int hh_far_apply(hh_ctx* ctx) {
       }
       continue;
     }
-    if (c == 0 && ctx->far_impl == FAR_MID_IMPL && ctx->mid_bound < e) {
+    if (c == 0 && ctx->far_impl == 0 && ctx->mid_bound < e) {
       // mid-size blocks [max(b, mid_bound), e): whole blocks per persistent CTA, rank by rank through the ring
       const u32 mb = ctx->mid_bound > b ? ctx->mid_bound : b;
       const size_t smem = (size_t)FAR_MID_RING + 128 + 2 * FAR_NS * 8 + FAR_NS * sizeof(FarMidDesc) + FAR_NS * 4 + 2 * HH_MAX_RANK * 16 * 4;

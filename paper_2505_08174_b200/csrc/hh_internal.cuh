@@ -56,6 +56,8 @@ struct DevScalars {
   u64 fallback_entries;
   u64 n_self_pairs;         /* pairs (i, j in N(i)) visited by the two-body self term */
   u64 cap_count;            /* pivot records written by hh_set_capture's kernel (may exceed the caller's capacity) */
+  u32 batch_mid;            /* lock-step ACA, two half-batches in flight: first block of the second half (half of the rows + columns each) */
+  u32 ab[6];                /* per half: active blocks [0,1], row granules [2,3], column granules [4,5]                     */
   u64 batch_units, batch_units1;  /* lock-step ACA: padded rows + columns of the batch [first, batch_end) resp. of block `first` alone */
 };
 
@@ -85,6 +87,8 @@ struct hh_ctx {
   /* pinned host scratch */
   DevScalars* h_sc;
   cudaEvent_t ev[8];
+  cudaStream_t stream2;                 /* side stream of the two-half lock-step ACA (hh_set_aca_impl 4): carries the update kernel of one half while the other half's entries are evaluated */
+  cudaEvent_t ev_ab[2];
   /* carved device pointers */
   DevScalars* d_sc;
   float *w2, *w3;                       /* packed weights                                     */

@@ -207,7 +207,7 @@ def test_far_ring_kernel_equals_one_cta_per_block(mlp2, leaf, n, eta, tol):
     """row 9, both forms on the SAME resident factors: the ring kernel (persistent CTAs, TMA bulk copies into a shared-memory
     byte ring; blocks with max(m,n) <= 256) against round 1's one-CTA-per-block kernel, in every ring size class (leaf 200:
     129..256, leaf 100: 65..128, leaf 40: <= 64, leaf 3: rows and columns below the pad width, ranks up to min(m,n)) and the
-    whole-block ring kernel k_far_mid (hh_set_far_impl 2) for 256 < max(m,n) <= 1024 (40,000 and 30,000 particles: blocks of
+    whole-block ring kernel k_far_mid for 256 < max(m,n) <= 1024 (40,000 and 30,000 particles: blocks of
     300..1,000 rows, several chunks per block)"""
     X = synth.ball_cloud(n, 0.2, seed=11) if leaf != 40 else synth.chain_cloud(n // 50, 50, 0.1)
     F = synth.gaussian_forces(len(X), seed=3)
@@ -223,7 +223,7 @@ def test_far_ring_kernel_equals_one_cta_per_block(mlp2, leaf, n, eta, tol):
         ctx.set_far_impl(0)
         U0 = ctx.far_apply_resident(to_dev(F)).cpu().numpy()
         U0b = ctx.far_apply_resident(to_dev(F)).cpu().numpy()      # the item list is reused while the factors stay resident
-        ctx.set_far_impl(2)                                         # + k_far_mid for 256 < max(m,n) <= 1024
+        ctx.set_far_impl(2)                                         # without k_far_mid (256 < max(m,n) <= 1024 by one CTA per block)
         U2 = ctx.far_apply_resident(to_dev(F)).cpu().numpy()
         assert np.linalg.norm(U1) > 0
         worst = max(worst, rel_l2(U0, U1), rel_l2(U0b, U1), rel_l2(U2, U1))
@@ -287,13 +287,14 @@ def test_degenerate_blocks(mlp2):
 
 def test_both_aca_forms_agree(mlp2):
     """hh_set_aca_impl: the lock-step forms (0, the default: entries and vectorised update in separate launches; 2: stored terms
-    staged by TMA bulk copies; 3: entries and update fused) and the one-CTA-per-block form (1) run the same Alg. 2; pivots, ranks
+    staged by TMA bulk copies; 3: entries and update fused; 4: form 0 on two half-batches one listing line apart, the update of one
+    beside the entry evaluation of the other) and the one-CTA-per-block form (1) run the same Alg. 2; pivots, ranks
     and flags agree on all but near-tie blocks and the mat-vecs agree to fp32 summation order.  The lock-step forms do the same
     arithmetic in the same order on each entry (only the Gram sums are float atomics), so they differ by even less."""
     X = synth.cube_cloud(5000, 0.1, seed=9)
     F = synth.gaussian_forces(5000)
     res = []
-    for impl in (0, 1, 2, 3):
+    for impl in (0, 1, 2, 3, 4):
         ctx = setup(X, mlp2, leaf_size=32, eta=1.0, aca_tol=1e-4, ws_mb=8192)
         ctx.set_aca_impl(impl)
         U = ctx.matvec(to_dev(F)).cpu().numpy()
@@ -301,7 +302,7 @@ def test_both_aca_forms_agree(mlp2):
         res.append((U, ranks, flags, ctx.stats()))
         ctx.close()
     U0, r0, f0, s0 = res[0]
-    for impl in (1, 2, 3):
+    for impl in (1, 2, 3, 4):
         U1, r1, f1, s1 = res[impl]
         assert s0["aca_batches"] == s1["aca_batches"] == 1
         print("aca_impl %d vs 0: rel L2 %.3e, ranks differ on %.4f of the blocks" % (impl, rel_l2(U0, U1), np.mean(r0 != r1)))
@@ -310,7 +311,7 @@ def test_both_aca_forms_agree(mlp2):
         assert rel_l2(U0, U1) <= 1e-5
 
 
-IMPLS = (0, 2, 3)
+IMPLS = (0, 2, 3, 4)
 
 
 @pytest.mark.parametrize("name,gen,leaf,eta,zeta", [

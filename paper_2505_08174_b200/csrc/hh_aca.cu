@@ -410,6 +410,7 @@ int hh_aca_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   cudaStream_t s = ctx->stream;
   const u32 nG = (u32)ctx->nG;
   // the table (one 128-B row per resident block) sits at the start of the scratch region, the arena after it
+  if (first == 0) ctx->l_pred = ctx->l_pred_first;
   u32 chunks_pred = (u32)((ctx->l_pred + HH_RC - 1) / HH_RC);
   if (chunks_pred < 1) chunks_pred = 1;
   if (chunks_pred > HH_MAX_CHUNKS) chunks_pred = HH_MAX_CHUNKS;
@@ -510,6 +511,7 @@ int hh_aca_batch_finish(hh_ctx* ctx, int64_t first, u32 end, int64_t* next) {
     double pred = (mean_rank + HH_RC) * 1.10;
     if (h.fail_min < end) pred = ctx->l_pred * 1.25 > pred ? ctx->l_pred * 1.25 : pred;
     ctx->l_pred = pred < HH_RC ? HH_RC : (pred > HH_MAX_RANK ? HH_MAX_RANK : pred);
+    if (first == 0) ctx->l_pred_first = ctx->l_pred;
   }
   return HH_OK;
 }

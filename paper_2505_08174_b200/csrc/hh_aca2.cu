@@ -21,6 +21,9 @@
 // Storage, arena chunks, table rows and the pivot record are those of hh_aca.cu (the far-field kernel reads both).
 #include "hh_mlp.cuh"
 #include "hh_wide.cuh"
+#ifdef HH_PROF
+#include <chrono>
+#endif
 
 #define GR 16                    /* entries per granule = half a warp                                   */
 #define A2_T 256                 /* threads of the entry-evaluating kernels                              */
@@ -1203,6 +1206,7 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
   cudaStream_t s = ctx->stream;
   const u32 nG = (u32)ctx->nG;
   const int R = ctx->p.aca_max_rank;
+  if (first == 0) ctx->l_pred = ctx->l_pred_first;
   u32 chunks_pred = (u32)((ctx->l_pred + HH_RC - 1) / HH_RC);
   if (chunks_pred < 1) chunks_pred = 1;
   if (chunks_pred > HH_MAX_CHUNKS) chunks_pred = HH_MAX_CHUNKS;
@@ -1263,6 +1267,9 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     const unsigned gb = cdiv(nb, 256);
     k2_init<<<HH_N + gb, 256, 0, s>>>(A);
     HH_LAUNCH_CHECK();
+#ifdef HH_PROF
+    double prof_sync = 0, prof_launch = 0; int prof_it = 0; auto prof_last = std::chrono::steady_clock::now(); const auto prof_t0 = prof_last;
+#endif
     if (two_halves) HH_TRY(a2_two_halves(ctx, A, ctx->h_sc->batch_mid, cm2, cn2, gm2, gn2, ngran));
     else
     for (int it = 0; it <= R; ++it) {
@@ -1272,7 +1279,14 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
       HH_TRY(hh_scan_u32(ctx, A.cn, A.cn, nb, &ctx->d_sc->lvl.h));
       HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->n_split, &ctx->d_sc->n_split, sizeof(u32), cudaMemcpyDeviceToHost, s));
       HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->lvl, &ctx->d_sc->lvl, sizeof(Cnt3), cudaMemcpyDeviceToHost, s));
+#ifdef HH_PROF
+      const auto tp0 = std::chrono::steady_clock::now();
+#endif
       HH_CUDA(cudaStreamSynchronize(s));
+#ifdef HH_PROF
+      { const auto tp1 = std::chrono::steady_clock::now(); prof_sync += std::chrono::duration<double, std::milli>(tp1 - tp0).count();
+        prof_launch += std::chrono::duration<double, std::milli>(tp0 - prof_last).count(); prof_last = tp1; ++prof_it; }
+#endif
       const u32 nact = ctx->h_sc->n_split, gmc = ctx->h_sc->lvl.g, gnc = ctx->h_sc->lvl.h;
       if (nact == 0) break;
       if (gmc > ngran || gnc > ngran) return hh_fail(ctx, HH_ERR_CUDA, "lock-step ACA: granule list overflow (internal)");
@@ -1325,6 +1339,10 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
     // in the batch.  Then most of the batch would be discarded -- shrink the batch and run it again instead.
     HH_CUDA(cudaMemcpyAsync(&ctx->h_sc->fail_min, &ctx->d_sc->fail_min, sizeof(u32), cudaMemcpyDeviceToHost, s));
     HH_CUDA(cudaStreamSynchronize(s));
+#ifdef HH_PROF
+    fprintf(stderr, "[HH_PROF] batch first=%lld nb=%u: %d iterations, wall %.1f ms, host waiting in sync %.1f ms, host between syncs (launching) %.1f ms\n", (long long)first, nb,
+            prof_it, std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - prof_t0).count(), prof_sync, prof_launch);
+#endif
     const u32 fm = ctx->h_sc->fail_min;
     if (fm < end && nb > 1 && (fm - (u32)first) < nb - nb / 4) {
       end_cap = (u32)first + (nb / 2 > 1 ? nb / 2 : 1);

@@ -169,7 +169,7 @@ extern "C" int hh_create(hh_ctx** out, const hh_params* params, const hh_mlp* ml
   ctx->ws = (char*)workspace;
   ctx->ws_bytes = workspace_bytes;
   ctx->pairs_per_particle = 32;
-  ctx->l_pred = 32.0;
+  ctx->l_pred = ctx->l_pred_first = 32.0;
   *out = ctx;
   {
     int dev = 0, nsm = 0;
@@ -249,7 +249,7 @@ extern "C" int hh_set_params(hh_ctx* ctx, const hh_params* params) {
   if (params->eta != ctx->p.eta) ctx->blocks_ok = 0;
   ctx->res_first = ctx->res_next = 0;               // factors depend on tol / rank cap / rule / kappa_max
   ctx->n_dense = 0;
-  ctx->l_pred = 32.0;
+  ctx->l_pred = ctx->l_pred_first = 32.0;
   ctx->p = *params;
   return HH_OK;
 }

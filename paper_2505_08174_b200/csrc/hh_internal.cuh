@@ -80,6 +80,9 @@ struct hh_ctx {
   int64_t nG, nH, cap_pairs;
   int64_t res_first, res_next;          /* resident factor range [first, next) of sorted P^G */
   double l_pred;                        /* predicted rank for batch sizing                   */
+  double l_pred_first;                  /* what the FIRST batch of a mat-vec (the largest blocks) needed last time: the next mat-vec starts from it
+                                           instead of the last batch's prediction (leaf-size blocks, half the rank), which made every step's first batch
+                                           overflow the arena and run twice (c3: 750 ms of a 5.4 s step) */
   u32 class_bound[5];
   u32 mid_bound;                        /* first block of sorted P^G with max(m,n) <= HH_FAR_MID_MAX */
   hh_stats st;

@@ -6,18 +6,20 @@
 // iteration form one flat, load-balanced work list, and the MLP is evaluated in registers exactly as in the
 // near-field kernel (hh_mlp.cuh).  A 2^19-row top-level block and a 20-row leaf block cost the same per entry.
 //
-// One iteration k (all blocks in lock step; blocks drop out as they stop):
-//   (k_col = k2_step<false>, k_row = k2_step<true>: entry evaluation and update fused, stored terms prefetched into L2)
-//   k_col   line 4-5  c'(i) = G(i,j_k) - sum_p C_p(i) Q_p(j_k), stored raw; arg-max scores (Eq. (9), S-18) by atomicMax;
-//                     A'_pk = sum_i C_p(i)^T c'(i)
-//   k_piv   line 5-6  pivot row i_k, P = c'(i_k), P^-1 and cond_F(P) in fp64; zero column -> done (S-21); singular or
-//                     cond_F > kappa_max -> breakdown, block goes dense (S-18, S-18b); A_pk = A'_pk P^-1
-//   (line 6)          c_k(i) = c'(i) P^-1 (fp64 products, rounded once); A_kk = sum_i c_k(i)^T c_k(i)   (S-19);
-//                     memory-bound, interleaved with the MLP tiles of the row side inside k2_step<true>
-//   k_row   line 7-8  q_k(j) = G(i_k,j) - sum_p C_p(i_k) Q_p(j), stored raw; arg-max for j_{k+1};
-//                     B_kk = sum_j q(j) q(j)^T, cross = sum_j tr([sum_p Q_p(j)^T A_pk] q(j))  (= sum_p tr(A_pk B_kp), S-19)
-//   k_fin   line 9-12 nu^2 = tr(A_kk B_kk); lambda^2 += nu^2 + 2 cross; stop test Eq. (10) (S-20);
-//                     next column; arena space for the next HH_RC ranks
+// One iteration k (all blocks in lock step; blocks drop out as they stop), the default form (hh_set_aca_impl 0):
+//   k2_eval<rows>    line 4    raw entries G(i, j_k) into the slot of rank k (the MLP, two entries per thread)
+//   k2_upd<rows>     line 4-5  c'(i) = G(i,j_k) - sum_p C_p(i) Q_p(j_k) (4 rows per thread, vector loads); arg-max scores
+//                              (Eq. (9), S-18) by atomicMax; A'_pk = sum_i C_p(i)^T c'(i)
+//   k2_piv           line 5-6  pivot row i_k, P = c'(i_k), P^-1 and cond_F(P) in fp64; zero column -> done (S-21); singular or
+//                              cond_F > kappa_max -> breakdown, block goes dense (S-18, S-18b); A_pk = A'_pk P^-1
+//   k2_eval<columns> line 7    raw entries G(i_k, j); and line 6 rides along: c_k(i) = c'(i) P^-1 (fp64 products, rounded
+//                              once), A_kk = sum_i c_k(i)^T c_k(i) (S-19) -- memory-bound, hidden by this kernel's arithmetic
+//   k2_upd<columns>  line 7-8  q_k(j) = G(i_k,j) - sum_p C_p(i_k) Q_p(j) (2 columns per thread); arg-max for j_{k+1};
+//                              B_kk = sum_j q(j) q(j)^T, cross = sum_j tr([sum_p Q_p(j)^T A_pk] q(j))  (= sum_p tr(A_pk B_kp), S-19)
+//   k2_fin           line 9-12 nu^2 = tr(A_kk B_kk); lambda^2 += nu^2 + 2 cross; stop test Eq. (10) (S-20);
+//                              next column; arena space for the next HH_RC ranks
+// k2_step is the fused form (entries and update in one kernel; hh_set_aca_impl 3, and the fp64 parity mode), k2_step_t the
+// fused form with TMA-staged rank terms (2), a2_two_halves form 0 on two half-batches one listing line apart (4).
 // Storage, arena chunks, table rows and the pivot record are those of hh_aca.cu (the far-field kernel reads both).
 #include "hh_mlp.cuh"
 #include "hh_wide.cuh"

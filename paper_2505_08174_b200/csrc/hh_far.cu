@@ -1,7 +1,11 @@
 // hh_far.cu -- SURVEY 8(a) row 9, the roofline-graded kernel: far-field apply over the factors resident in
 // the arena, U^tau += C (Q F^sigma) per admissible block.  Bandwidth-bound: every
-// factor byte is read exactly once, as coalesced float4 (Q) / 128-B warp rows (C) from plane-major storage;
-// F^sigma is staged in shared memory tile by tile; t = Q F^sigma (3 floats per rank) never leaves the SM.
+// factor byte is read exactly once from plane-major storage; t = Q F^sigma (3 floats per rank) never leaves the SM.
+// Three kernels by block size (P^G is sorted by max(m,n), so each takes a contiguous range of a batch):
+//   k_far_ring  max(m,n) <= 256    persistent CTAs, arena chunks through a shared-memory ring filled by TMA bulk copies
+//   k_far_mid   257 .. 1024        the same ring, whole blocks per CTA, one bulk copy per rank's nine planes
+//   k_far       larger             one CTA per block, coalesced float4 (Q) / 128-B warp rows (C), F^sigma staged per tile
+// (hh_set_far_impl selects k_far for everything, or the ring only up to 256, for comparison.)
 #include "hh_internal.cuh"
 
 #define FAR_SUB 512            /* columns per (rank, sub-tile) warp work unit                 */

@@ -31,8 +31,8 @@ METRIC = "H-matvec particles/s (whole step: tree + blocks + ACA + near + far + t
 UNIT = "particles/s"
 FAR_BYTES_PER_UNIT = 36          # bytes of fp32 factors read per (row or column) x block-rank (DESIGN.md far-field)
 # dram__bytes_read.sum + dram__bytes_write.sum of the k_far launches / their algorithmic factor bytes, from the ncu --set full
-# capture summarised in profiles/r02_far_traffic_c3.md (per launch; the bench line scales it to the launches of one step)
-FAR_TRAFFIC_RATIO = 1.063
+# capture summarised in profiles/r02c_far_c3.md (per launch; the bench line scales it to the launches of one step)
+FAR_TRAFFIC_RATIO = 1.046
 ORACLE_SAMPLE_N = {"c1": 2048, "c2": 8192, "c3": 24576, "c4": 16384, "c5": 16000, "p1": 60000, "p2": 60000}
 
 
@@ -320,7 +320,7 @@ def run_gpu(args):
         "roofline": {"kernel": "k_far (far-field apply U^tau += C (Q F^sigma), all size classes and arena batches of one step)",
                      "bound": "hbm", "achieved": far_gbs, "peak": hbm_peak, "unit": "GB/s", "frac": far_gbs / hbm_peak,
                      "traffic": FAR_TRAFFIC_RATIO * far_bytes if FAR_TRAFFIC_RATIO else None,
-                     "traffic_note": "dram bytes of the k_far launches of one step = ncu-measured ratio x algorithmic bytes (profiles/r02_far_traffic_c3.md); not re-collected in this run",
+                     "traffic_note": "dram bytes of the k_far launches of one step = ncu-measured ratio x algorithmic bytes (profiles/r02c_far_c3.md); not re-collected in this run",
                      "peak_source": peak_src, "share_of_step": far_ms / step_ms,
                      "algorithmic_bytes_per_step": far_bytes, "ms_per_step": far_ms},
         "wall_s_timed_region": t_wall,

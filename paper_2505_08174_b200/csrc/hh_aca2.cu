@@ -1346,6 +1346,9 @@ int hh_aca2_batch(hh_ctx* ctx, int64_t first, int64_t* next) {
             prof_it, std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - prof_t0).count(), prof_sync, prof_launch);
 #endif
     const u32 fm = ctx->h_sc->fail_min;
+#ifdef HH_PROF
+    fprintf(stderr, "[HH_PROF]   fail_min %u of [%lld, %u): %s, l_pred %.1f\n", fm, (long long)first, end, fm < end ? "OVERFLOW" : "fits", ctx->l_pred);
+#endif
     if (fm < end && nb > 1 && (fm - (u32)first) < nb - nb / 4) {
       end_cap = (u32)first + (nb / 2 > 1 ? nb / 2 : 1);
       ctx->l_pred = ctx->l_pred * 1.25 > HH_MAX_RANK ? HH_MAX_RANK : ctx->l_pred * 1.25;

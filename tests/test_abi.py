@@ -60,3 +60,27 @@ def test_no_cpu_fallback_without_a_device():
         assert "CUDA" in str(e)
     else:
         raise AssertionError("Context() must raise without a CUDA device")
+
+
+def test_static_entry_point_checks_its_arguments_without_a_device():
+    """hh_dense_matvec_static (the entry point that allocates nothing): size limit and argument errors come with a text before
+    any CUDA call is made; with plausible arguments and no device it fails with HH_ERR_CUDA (no CPU fallback)."""
+    import torch
+    import paper_2505_08174_b200 as hh
+    lib = hh.load()
+    dims = (C.c_int32 * 4)(4, 32, 32, 9)
+    one = C.c_void_p(256)                         # non-null, never dereferenced on these paths
+    pw = (C.c_void_p * 3)(256, 256, 256)
+    mlp = hh._Mlp(3, dims, pw, pw)
+    err = C.create_string_buffer(256)
+
+    def call(n, m=mlp, x=one):
+        return lib.hh_dense_matvec_static(C.byref(m), C.c_float(1.0), x, one, one, C.c_int64(n), None, err, C.c_size_t(256))
+
+    assert call(hh.STATIC_MAX_N + 1) == -2 and b"HH_STATIC_MAX_N" in err.value
+    assert call(0) == -1 and b"N < 1" in err.value
+    assert call(10, x=None) == -1
+    bad = hh._Mlp(3, (C.c_int32 * 4)(7, 64, 64, 9), pw, pw)
+    assert call(10, m=bad) == -5 and b"4-32-32-9" in err.value
+    if not torch.cuda.is_available():
+        assert call(10) == -3 and b"hh_dense_matvec_static" in err.value

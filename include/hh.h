@@ -128,8 +128,9 @@ int hh_set_params(hh_ctx* ctx, const hh_params* params);
 /* Alg. 2 form: 0 = lock-step over all blocks of an arena batch (default; each listing line a parallel pass over
  * the selected blocks), entry evaluation and the vectorised update as separate launches; 1 = one CTA per block; 2 = lock-step
  * with the stored rank terms of a tile of 256 rows staged through shared memory by TMA bulk copies; 3 = lock-step with entry
- * evaluation and update fused in one kernel.  1-3 are measured slower and kept for comparison.  Same factors up to fp32
- * summation order in the norm recursion. */
+ * evaluation and update fused in one kernel; 4 = form 0 on two half-batches one listing line apart (the update of one on a
+ * side stream beside the entry evaluation of the other).  1-4 are measured slower and kept for comparison.  Same factors up
+ * to fp32 summation order in the norm recursion. */
 int hh_set_aca_impl(hh_ctx* ctx, int impl);
 
 /* Far-field apply form: 0 = blocks with max(m,n) <= 1024 are streamed by persistent CTAs through a

@@ -263,7 +263,8 @@ extern "C" int hh_set_pair_capacity(hh_ctx* ctx, int64_t pairs_per_particle) {
 
 // 0 = lock-step over the batch, entries (k2_eval) and vectorised update (k2_upd) as separate launches (default),
 // 1 = one CTA per admissible block (the first form), 2 = lock-step with the stored terms staged through shared memory by TMA
-// bulk copies, 3 = lock-step with entries and update fused in one kernel (k2_step); 1-3 measured slower, kept for comparison
+// bulk copies, 3 = lock-step with entries and update fused in one kernel (k2_step), 4 = form 0 on two half-batches (a2_two_halves);
+// 1-4 measured slower, kept for comparison
 extern "C" int hh_set_aca_impl(hh_ctx* ctx, int impl) {
   if (!ctx || impl < 0 || impl > 4) return HH_ERR_INVALID_ARG;
   if (impl == 1 && ctx->mlp2_wide) return hh_fail(ctx, HH_ERR_UNSUPPORTED, "the paper-size MLP runs in the lock-step form only");
